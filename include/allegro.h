@@ -1,0 +1,124 @@
+/* allegro.h — C-ABI boundary of the B200-native Allegro energy+force hot path.
+ *
+ * What the calls compute is defined by PAPER.md:93 (Allegro hyper-parameters: tensor features, l,
+ * full O(3), two-body / latent / edge-energy MLPs, radial cutoff), Table 1,
+ * PAPER.md:29 (the architecture of the paper's ref. 22), PAPER.md:9 (strictly local, E(3)-equivariant)
+ * and PAPER.md:89/:116 (explicit reversible integrator, 0.48-0.5 fs steps), with every convention the
+ * paper leaves open fixed by the readings A1-A24 of SURVEY.md section 8c (listed in DESIGN.md).
+ *
+ * Conventions
+ *  - Every function returns an int status: ALLEGRO_OK (0) or a negative ALLEGRO_ERR_* code.  No C++
+ *    exception crosses the boundary.  allegro_last_error(h) returns a NUL-terminated message owned by
+ *    the handle (valid until the next call on that handle); with h == NULL it returns the message of
+ *    the last failed allegro_create on this thread.
+ *  - Pointers marked DEVICE are CUDA device pointers, pointers marked HOST are host pointers.  The
+ *    caller owns every array it passes; the library never frees nor retains a caller pointer past the
+ *    call.  The handle owns all internal device buffers (neighbour list, workspaces, MD state).
+ *  - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Work is enqueued on that
+ *    stream; allegro_build_neighbors, allegro_energy_forces, allegro_md_step and the get_* calls
+ *    synchronise the stream once before returning so that the status reflects device-side error flags.
+ *    There is no host synchronisation inside the step loop of allegro_md_step except the one-word
+ *    read-back that sizes a rebuilt neighbour list.
+ *  - Units: Angstrom, fs, amu, eV.  Positions / velocities / masses / cell are fp64; the network runs
+ *    in fp32.  Cells are orthorhombic (row vectors, off-diagonals must be 0) — triclinic cells return
+ *    ALLEGRO_ERR_UNSUPPORTED.
+ *  - There is no CPU fallback: without a CUDA device every compute call returns ALLEGRO_ERR_CUDA.
+ */
+#ifndef ALLEGRO_B200_H
+#define ALLEGRO_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  ALLEGRO_OK = 0,
+  ALLEGRO_ERR_INVALID = -1,      /* bad argument / hyper-parameters / weight count                   */
+  ALLEGRO_ERR_UNSUPPORTED = -2,  /* non-orthorhombic cell, lmax > 3, a row longer than the kernel cap  */
+  ALLEGRO_ERR_CUDA = -3,         /* CUDA runtime error (message has the cudaGetErrorString text)       */
+  ALLEGRO_ERR_STALE_LIST = -4,   /* some atom moved more than skin/2 since allegro_build_neighbors     */
+  ALLEGRO_ERR_NONFINITE = -5,    /* NaN/Inf detected in E or F                                         */
+  ALLEGRO_ERR_CUTOFF = -6,       /* r_cut + skin exceeds the smallest box length (reading A17)         */
+  ALLEGRO_ERR_SPECIES = -7,      /* a species index outside [0, n_species)                             */
+  ALLEGRO_ERR_NO_LIST = -8,      /* energy_forces / get_neighbors before build_neighbors               */
+  ALLEGRO_ERR_ALLOC = -9         /* device allocation failed                                           */
+};
+
+/* kinds of tensors in the weight blob, as reported by allegro_weight_layout */
+enum { ALLEGRO_WK_MATRIX = 0, ALLEGRO_WK_RESIDUAL = 1, ALLEGRO_WK_SIGMA = 2, ALLEGRO_WK_MU = 3 };
+
+/* Hyper-parameters (Table 1).  *_dims lists the output width of each linear layer of the
+ * MLP ("dimensions [a,b,c]" = in->a->b->c with SiLU between, none after the last, no biases: A5); the
+ * last two_body and latent widths must both equal the latent width D (A10).  edge_dims are the hidden
+ * widths of the edge-energy MLP (no non-linearity, final ->1 implicit).  full_o3 = 1 is the paper's
+ * "full O(3) symmetry"; 0 keeps only paths with l1+l2+lo even. */
+typedef struct {
+  int32_t n_species, n_bessel, poly_p, lmax, n_layers, n_channels, full_o3;
+  int32_t two_body_nl, two_body_dims[8];
+  int32_t latent_nl, latent_dims[8];
+  int32_t edge_nl, edge_dims[8];
+  double r_cut, avg_num_neighbors;
+} allegro_hparams;
+
+/* Layout of the flat fp32 weight blob for `hp` (SURVEY.md 8b "Weight blob order"): tensor t has
+ * kind[t] (ALLEGRO_WK_*), rows[t] x cols[t] values, row-major [out,in], tensors concatenated in order.
+ * Returns the number of tensors (>= 0) or a negative error; writes at most `max_tensors` entries
+ * (arrays may be NULL to query the count only).  HOST pointers.  Pure host logic, no CUDA needed. */
+int allegro_weight_layout(const allegro_hparams* hp, int32_t* kind, int64_t* rows, int64_t* cols, int max_tensors);
+
+/* Build a model: validates hp, derives the irreps/path plan and the real coupling tables, copies the
+ * weights (HOST pointer, n_weights floats in blob order) to the device.  *handle_out receives the handle. */
+int allegro_create(const float* weights_host, size_t n_weights, const allegro_hparams* hp, void** handle_out);
+int allegro_destroy(void* h);
+
+/* Row a-1: device cell-list neighbour builder.  pos DEVICE fp64 [N,3] (unwrapped), species DEVICE int32
+ * [N], cell HOST fp64 [3,3].  Builds the sorted CSR list of all ordered (i, j, s) with
+ * |r_j + s.cell - r_i|^2 < (cutoff+skin)^2 evaluated in fp64 as dx = (x_j-x_i)+s_x*L_x, d2=dx*dx+dy*dy+dz*dz
+ * (A16), (i,j,s) != (i,i,0), each row sorted by (j, sx, sy, sz).  cutoff must equal hp.r_cut. */
+int allegro_build_neighbors(void* h, const double* pos, const int32_t* species, int64_t N,
+                            const double* cell, double cutoff, double skin, void* stream);
+
+/* Rows a-2..a-5: energy and forces with the list of the last allegro_build_neighbors.
+ * E_out DEVICE fp64 [1]; F_out DEVICE fp64 [N,3]; E_atom_out DEVICE fp32 [N] or NULL.
+ * Returns ALLEGRO_ERR_STALE_LIST (outputs undefined) if an atom moved more than skin/2 since the build
+ * (with skin = 0 any displacement is stale); it never rebuilds silently. */
+int allegro_energy_forces(void* h, const double* pos, const int32_t* species, int64_t N, const double* cell,
+                          double* E_out, double* F_out, float* E_atom_out, void* stream);
+
+/* Row a-6: velocity-Verlet NVE (kick-drift-kick, A20), state kept inside the handle.
+ * md_init copies pos/vel/mass/species (DEVICE), builds the list and evaluates the initial forces.
+ * md_step advances n_steps; after each drift it rebuilds the list when max_i |r_i - r_i^build| > skin/2
+ * (skin = 0: every step, A22). */
+int allegro_md_init(void* h, const double* pos, const double* vel, const double* mass, const int32_t* species,
+                    int64_t N, const double* cell, double cutoff, double skin, void* stream);
+int allegro_md_step(void* h, double dt_fs, int64_t n_steps, void* stream);
+
+/* Copies the MD state out.  pos/vel/F DEVICE fp64 [N,3]; E_pot/E_kin DEVICE fp64 [1]; n_rebuilds HOST
+ * int64 [1].  Any pointer may be NULL. */
+int allegro_get_state(void* h, double* pos, double* vel, double* F, double* E_pot, double* E_kin,
+                      int64_t* n_rebuilds, void* stream);
+
+/* Copies the current list out.  E_list HOST int64 [1] is always written (call with the arrays NULL to
+ * size them); rowptr DEVICE int64 [N+1], col DEVICE int32 [E_list], shift DEVICE int8 [E_list,3]. */
+int allegro_get_neighbors(void* h, int64_t* rowptr, int32_t* col, int8_t* shift, int64_t* E_list);
+
+/* Counters of the last energy_forces / md_step call (HOST int64 [8]): [0] active edges (r < r_cut) of
+ * the last force evaluation, [1] list edges, [2] kernel launches of the call, [3] rebuilds of the call,
+ * [4] force evaluations of the call, [5..7] reserved. */
+int allegro_get_stats(void* h, int64_t* stats);
+
+/* Debug taps for the CPU-only tests (pure host logic, no CUDA): the library's own real coupling tensor
+ * C^(l1 l2 l3) (reading A9), dense row-major [2l1+1][2l2+1][2l3+1] into out (HOST, fp64); and the number of
+ * tensor-product paths of layer L (1-based) of the plan derived from hp.  Negative return = error. */
+int allegro_debug_coupling(int l1, int l2, int l3, double* out);
+int allegro_debug_num_paths(const allegro_hparams* hp, int layer);
+
+const char* allegro_last_error(void* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ALLEGRO_B200_H */

@@ -1,0 +1,214 @@
+"""Thin ctypes binding over the C-ABI of include/allegro.h (argument marshalling only).
+
+Every step of the hot path runs in the CUDA kernels of liballegro_b200.so; torch is used here only
+for device memory and streams.  There is no CPU fallback: importing this module raises if the shared
+library has not been built (``python -m paper_2502_06073_b200.build``), and every compute call raises
+``AllegroError`` when the library reports an error (e.g. no CUDA device).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liballegro_b200.so")
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_2502_06073_b200.build` "
+                      "(the CUDA extension is required; there is no CPU fallback)")
+_lib = C.CDLL(LIB_PATH)
+
+ERR_NAMES = {0: "OK", -1: "INVALID", -2: "UNSUPPORTED", -3: "CUDA", -4: "STALE_LIST", -5: "NONFINITE", -6: "CUTOFF",
+             -7: "SPECIES", -8: "NO_LIST", -9: "ALLOC"}
+EXPORTS = ["allegro_weight_layout", "allegro_create", "allegro_destroy", "allegro_build_neighbors",
+           "allegro_energy_forces", "allegro_md_init", "allegro_md_step", "allegro_get_state",
+           "allegro_get_neighbors", "allegro_get_stats", "allegro_debug_coupling", "allegro_debug_num_paths",
+           "allegro_last_error"]
+
+
+class HParams(C.Structure):
+    _fields_ = [("n_species", C.c_int32), ("n_bessel", C.c_int32), ("poly_p", C.c_int32), ("lmax", C.c_int32),
+                ("n_layers", C.c_int32), ("n_channels", C.c_int32), ("full_o3", C.c_int32),
+                ("two_body_nl", C.c_int32), ("two_body_dims", C.c_int32 * 8),
+                ("latent_nl", C.c_int32), ("latent_dims", C.c_int32 * 8),
+                ("edge_nl", C.c_int32), ("edge_dims", C.c_int32 * 8),
+                ("r_cut", C.c_double), ("avg_num_neighbors", C.c_double)]
+
+
+class AllegroError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"allegro error {code} ({ERR_NAMES.get(code, '?')}): {msg}")
+        self.code = code
+
+
+_vp, _i64, _dbl = C.c_void_p, C.c_int64, C.c_double
+_lib.allegro_weight_layout.argtypes = [C.POINTER(HParams), _vp, _vp, _vp, C.c_int]
+_lib.allegro_create.argtypes = [_vp, C.c_size_t, C.POINTER(HParams), C.POINTER(_vp)]
+_lib.allegro_destroy.argtypes = [_vp]
+_lib.allegro_build_neighbors.argtypes = [_vp, _vp, _vp, _i64, _vp, _dbl, _dbl, _vp]
+_lib.allegro_energy_forces.argtypes = [_vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _vp]
+_lib.allegro_md_init.argtypes = [_vp, _vp, _vp, _vp, _vp, _i64, _vp, _dbl, _dbl, _vp]
+_lib.allegro_md_step.argtypes = [_vp, _dbl, _i64, _vp]
+_lib.allegro_get_state.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]
+_lib.allegro_get_neighbors.argtypes = [_vp, _vp, _vp, _vp, _vp]
+_lib.allegro_get_stats.argtypes = [_vp, _vp]
+_lib.allegro_debug_coupling.argtypes = [C.c_int, C.c_int, C.c_int, _vp]
+_lib.allegro_debug_num_paths.argtypes = [C.POINTER(HParams), C.c_int]
+_lib.allegro_last_error.argtypes = [_vp]
+_lib.allegro_last_error.restype = C.c_char_p
+for _n in EXPORTS[:-1]:
+    getattr(_lib, _n).restype = C.c_int
+
+
+def make_hparams(hp: dict) -> HParams:
+    h = HParams()
+    for k in ("n_species", "n_bessel", "poly_p", "lmax", "n_layers", "n_channels", "full_o3"):
+        setattr(h, k, int(hp[k]))
+    for name in ("two_body", "latent", "edge"):
+        dims = list(hp[name + "_dims"])
+        if len(dims) > 8:
+            raise ValueError("at most 8 layers per MLP")
+        setattr(h, name + "_nl", len(dims))
+        arr = getattr(h, name + "_dims")
+        for i, d in enumerate(dims):
+            arr[i] = int(d)
+    h.r_cut = float(hp["r_cut"])
+    h.avg_num_neighbors = float(hp["avg_num_neighbors"])
+    return h
+
+
+def _last_error(handle=None) -> str:
+    s = _lib.allegro_last_error(handle)
+    return s.decode() if s else ""
+
+
+def allegro_weight_layout(hp: dict):
+    """-> list of (kind, rows, cols) in blob order."""
+    h = make_hparams(hp)
+    n = _lib.allegro_weight_layout(C.byref(h), None, None, None, 0)
+    if n < 0:
+        raise AllegroError(n, _last_error())
+    kind = np.zeros(n, np.int32); rows = np.zeros(n, np.int64); cols = np.zeros(n, np.int64)
+    _lib.allegro_weight_layout(C.byref(h), kind.ctypes.data, rows.ctypes.data, cols.ctypes.data, n)
+    return [(int(k), int(r), int(c)) for k, r, c in zip(kind, rows, cols)]
+
+
+def allegro_debug_coupling(l1, l2, l3) -> np.ndarray:
+    out = np.zeros((2 * l1 + 1, 2 * l2 + 1, 2 * l3 + 1))
+    rc = _lib.allegro_debug_coupling(l1, l2, l3, out.ctypes.data)
+    if rc < 0:
+        raise AllegroError(rc, "bad (l1,l2,l3)")
+    return out
+
+
+def allegro_debug_num_paths(hp: dict, layer: int) -> int:
+    h = make_hparams(hp)
+    rc = _lib.allegro_debug_num_paths(C.byref(h), layer)
+    if rc < 0:
+        raise AllegroError(rc, _last_error())
+    return rc
+
+
+def _ptr(t):
+    return None if t is None else t.data_ptr()
+
+
+def _stream():
+    import torch
+    return torch.cuda.current_stream().cuda_stream
+
+
+class Allegro:
+    """One model handle.  Methods mirror the C entry points one to one."""
+
+    def __init__(self, weights: np.ndarray, hp: dict):
+        w = np.ascontiguousarray(weights, dtype=np.float32)
+        self.hp = dict(hp)
+        self._h = _vp()
+        h = make_hparams(hp)
+        rc = _lib.allegro_create(w.ctypes.data, w.size, C.byref(h), C.byref(self._h))
+        if rc != 0:
+            raise AllegroError(rc, _last_error())
+
+    def _check(self, rc):
+        if rc != 0:
+            raise AllegroError(rc, _last_error(self._h))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib.allegro_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    @staticmethod
+    def _cell_host(cell):
+        return np.ascontiguousarray(np.asarray(cell, dtype=np.float64).reshape(3, 3))
+
+    def build_neighbors(self, pos, species, cell, cutoff, skin):
+        c = self._cell_host(cell)
+        self._n_atoms = pos.shape[0]
+        self._check(_lib.allegro_build_neighbors(self._h, _ptr(pos), _ptr(species), pos.shape[0], c.ctypes.data,
+                                                 float(cutoff), float(skin), _stream()))
+
+    def energy_forces(self, pos, species, cell, E_out, F_out, E_atom_out=None):
+        c = self._cell_host(cell)
+        self._check(_lib.allegro_energy_forces(self._h, _ptr(pos), _ptr(species), pos.shape[0], c.ctypes.data,
+                                               _ptr(E_out), _ptr(F_out), _ptr(E_atom_out), _stream()))
+
+    def md_init(self, pos, vel, mass, species, cell, cutoff, skin):
+        c = self._cell_host(cell)
+        self._n_atoms = pos.shape[0]
+        self._check(_lib.allegro_md_init(self._h, _ptr(pos), _ptr(vel), _ptr(mass), _ptr(species), pos.shape[0],
+                                         c.ctypes.data, float(cutoff), float(skin), _stream()))
+
+    def md_step(self, dt_fs, n_steps):
+        self._check(_lib.allegro_md_step(self._h, float(dt_fs), int(n_steps), _stream()))
+
+    def get_state(self, pos=None, vel=None, F=None, E_pot=None, E_kin=None):
+        nreb = C.c_int64(0)
+        self._check(_lib.allegro_get_state(self._h, _ptr(pos), _ptr(vel), _ptr(F), _ptr(E_pot), _ptr(E_kin),
+                                           C.addressof(nreb), _stream()))
+        return int(nreb.value)
+
+    def get_neighbors(self):
+        """-> (rowptr int64 [N+1], col int32 [E], shift int8 [E,3]) as torch CUDA tensors."""
+        import torch
+        E = C.c_int64(0)
+        self._check(_lib.allegro_get_neighbors(self._h, None, None, None, C.addressof(E)))
+        n = self._n_atoms
+        rowptr = torch.empty(n + 1, dtype=torch.int64, device="cuda")
+        col = torch.empty(max(E.value, 1), dtype=torch.int32, device="cuda")
+        shift = torch.empty((max(E.value, 1), 3), dtype=torch.int8, device="cuda")
+        torch.cuda.synchronize()
+        self._check(_lib.allegro_get_neighbors(self._h, _ptr(rowptr), _ptr(col), _ptr(shift), C.addressof(E)))
+        return rowptr, col[: E.value], shift[: E.value]
+
+    def get_stats(self) -> dict:
+        s = np.zeros(8, np.int64)
+        self._check(_lib.allegro_get_stats(self._h, s.ctypes.data))
+        return dict(active_edges=int(s[0]), list_edges=int(s[1]), launches=int(s[2]), rebuilds=int(s[3]),
+                    force_evals=int(s[4]))
+
+    # convenience wrappers (allocation + marshalling only) ---------------------------------------
+    def compute(self, pos_np, species_np, cell, skin=0.0, want_atom=False):
+        """Host arrays in, host arrays out: build list + one energy/force evaluation."""
+        import torch
+        pos = torch.from_numpy(np.ascontiguousarray(pos_np, dtype=np.float64)).cuda()
+        sp = torch.from_numpy(np.ascontiguousarray(species_np, dtype=np.int32)).cuda()
+        self._n_atoms = pos.shape[0]
+        E = torch.zeros(1, dtype=torch.float64, device="cuda")
+        F = torch.zeros((pos.shape[0], 3), dtype=torch.float64, device="cuda")
+        Ea = torch.zeros(pos.shape[0], dtype=torch.float32, device="cuda") if want_atom else None
+        self.build_neighbors(pos, sp, cell, self.hp["r_cut"], skin)
+        self.energy_forces(pos, sp, cell, E, F, Ea)
+        out = (float(E.item()), F.cpu().numpy())
+        return out + ((Ea.cpu().numpy(),) if want_atom else ())
+
+
+def build_weights(hp: dict, seed: int) -> np.ndarray:
+    """Random-init blob (A24) using the layout reported by the library."""
+    from . import workloads
+    return workloads.make_weights(allegro_weight_layout(hp), hp, seed)

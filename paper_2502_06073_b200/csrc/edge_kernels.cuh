@@ -1,0 +1,350 @@
+// edge_kernels.cuh — per-edge and per-row (centre atom) kernels of the forward and backward pass.
+// Steps refer to SURVEY.md 8c (F1-F12, B1-B12); PAPER.md:93 / :9 are the paper passages behind them.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "device_math.cuh"
+#include "model.h"
+
+namespace allegro {
+
+struct ListView {
+  const int64_t* rowptr;   // [N+1] list rows
+  const uint64_t* keys;    // [E_list] packed (j, s)
+  const int* revpos;       // [E_list]
+  double L[3];
+};
+
+__device__ __forceinline__ void decode_key(uint64_t key, int* j, int* sx, int* sy, int* sz) {
+  *j = (int)(key >> 24);
+  *sx = (int)((key >> 16) & 255) - 128; *sy = (int)((key >> 8) & 255) - 128; *sz = (int)(key & 255) - 128;
+}
+
+__device__ __forceinline__ double edge_d2(const double* __restrict__ pos, int64_t i, uint64_t key, const double* L,
+                                          double* dx, double* dy, double* dz, int* jout) {
+  int j, sx, sy, sz;
+  decode_key(key, &j, &sx, &sy, &sz);
+  *jout = j;
+  // A16: same expression order as the list criterion, fp64, no FMA contraction
+  *dx = __dadd_rn(__dsub_rn(pos[3 * (int64_t)j], pos[3 * i]), __dmul_rn((double)sx, L[0]));
+  *dy = __dadd_rn(__dsub_rn(pos[3 * (int64_t)j + 1], pos[3 * i + 1]), __dmul_rn((double)sy, L[1]));
+  *dz = __dadd_rn(__dsub_rn(pos[3 * (int64_t)j + 2], pos[3 * i + 2]), __dmul_rn((double)sz, L[2]));
+  return __dadd_rn(__dadd_rn(__dmul_rn(*dx, *dx), __dmul_rn(*dy, *dy)), __dmul_rn(*dz, *dz));
+}
+
+// stale-list test (A22) + species range check: one thread per atom
+__global__ void k_check_inputs(const double* __restrict__ pos, const double* __restrict__ r_build, const int* __restrict__ species,
+                               int64_t N, double half_skin2, int n_species, int* flags) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  double dx = pos[3 * i] - r_build[3 * i], dy = pos[3 * i + 1] - r_build[3 * i + 1], dz = pos[3 * i + 2] - r_build[3 * i + 2];
+  double d2 = dx * dx + dy * dy + dz * dz;
+  if (d2 > half_skin2) flags[FLAG_STALE] = 1;
+  int z = species[i];
+  if (z < 0 || z >= n_species) flags[FLAG_SPECIES] = 1;
+}
+
+// a-2 (first half): active-edge compaction (A11: edges with r >= r_c contribute exactly zero and are dropped).
+// One warp per centre atom of the chunk [a0, a1).  MODE 0 counts, MODE 1 fills the chunk-local edge arrays,
+// computes the edge geometry in fp64 (rounded to fp32 once) and zeroes g_list for the inactive list edges.
+template <int MODE>
+__global__ void k_active(const double* __restrict__ pos, const int* __restrict__ species, ListView lv, int64_t a0, int64_t a1,
+                         double rc, int poly_p, int n_bessel, int* __restrict__ act_cnt, const int64_t* __restrict__ rowptr_c,
+                         int* __restrict__ e_center, int* __restrict__ e_j, int64_t* __restrict__ e_lidx,
+                         float* __restrict__ geo, float* __restrict__ bes, float* __restrict__ g_list, int64_t cap_edges, int* flags) {
+  const int lane = threadIdx.x & 31;
+  const int64_t a = a0 + (((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
+  if (a >= a1) return;
+  const int64_t b = lv.rowptr[a], e = lv.rowptr[a + 1];
+  const double rc2 = rc * rc;
+  int total = 0;
+  const int64_t base = MODE ? rowptr_c[a - a0] : 0;
+  const int zi = MODE ? species[a] : 0;
+  for (int64_t k0 = b; k0 < e; k0 += 32) {
+    const int64_t k = k0 + lane;
+    bool act = false;
+    double dx = 0, dy = 0, dz = 0, d2 = 0;
+    int j = 0;
+    if (k < e) {
+      d2 = edge_d2(pos, a, lv.keys[k], lv.L, &dx, &dy, &dz, &j);
+      act = d2 < rc2;
+    }
+    const unsigned bal = __ballot_sync(0xffffffffu, act);
+    if (MODE == 1 && k < e) {
+      if (!act) {
+        g_list[3 * k] = 0.f; g_list[3 * k + 1] = 0.f; g_list[3 * k + 2] = 0.f;
+      } else {
+        const int64_t dst = base + total + __popc(bal & ((1u << lane) - 1u));
+        if (dst < cap_edges) {
+          const double r = sqrt(d2), inv = 1.0 / r;
+          const double x = r / rc;
+          double u, dudx;
+          envelope_d(x, poly_p, &u, &dudx);
+          e_center[dst] = (int)(a - a0);
+          e_j[dst] = j;
+          e_lidx[dst] = k;
+          float* gq = geo + dst * GEO_W;
+          gq[0] = (float)(dx * inv); gq[1] = (float)(dy * inv); gq[2] = (float)(dz * inv);
+          gq[3] = (float)r; gq[4] = (float)u; gq[5] = (float)(dudx / rc);
+          gq[6] = __int_as_float(zi); gq[7] = __int_as_float(species[j]);
+          // F2: b_n = (2/rc) sin(n pi r/rc)/r * u
+          const double pref = 2.0 / rc * inv * u, w = 3.14159265358979323846 * x;
+          for (int n = 1; n <= n_bessel; ++n) bes[dst * n_bessel + (n - 1)] = (float)(pref * sin(n * w));
+        } else {
+          flags[FLAG_ERR_CAP] = 2;
+        }
+      }
+    }
+    total += __popc(bal);
+  }
+  if (MODE == 0 && lane == 0) act_cnt[a - a0] = total;
+}
+
+// F7: Gamma_i[c, lm] = Nbar^-1/2 sum_{e in row(i)} w[e, c, l] Y_lm(rhat_e).  One block per centre atom; the
+// row's Y are staged in shared memory in slices of 32 edges; each thread owns outputs (c, lm) and sums the row
+// serially in CSR order (deterministic, no atomics).
+__global__ void k_gamma(const int64_t* __restrict__ rowptr_c, const float* __restrict__ geo, const float* __restrict__ w, int ldw,
+                        int n, int lmax, float inv_sqrt_navg, float* __restrict__ gamma, int64_t n_atoms) {
+  const int64_t a = blockIdx.x;
+  if (a >= n_atoms) return;
+  __shared__ float Ys[32][16];
+  const int dsh = (lmax + 1) * (lmax + 1), nout = n * dsh;
+  const int64_t b = rowptr_c[a], e = rowptr_c[a + 1];
+  constexpr int MAXO = 8;   // outputs per thread (n * d_sh <= 8 * blockDim)
+  float acc[MAXO];
+#pragma unroll
+  for (int q = 0; q < MAXO; ++q) acc[q] = 0.f;
+  for (int64_t k0 = b; k0 < e; k0 += 32) {
+    const int cnt = (int)min((int64_t)32, e - k0);
+    __syncthreads();
+    if (threadIdx.x < cnt) {
+      const float* gq = geo + (k0 + threadIdx.x) * GEO_W;
+      sph_harm_rt(lmax, gq[0], gq[1], gq[2], Ys[threadIdx.x]);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < MAXO; ++q) {
+      const int o = threadIdx.x + q * blockDim.x;
+      if (o < nout) {
+        const int c = o / dsh, lm = o - c * dsh;
+        const int l = (lm >= 9) ? 3 : (lm >= 4) ? 2 : (lm >= 1) ? 1 : 0;
+        float s = 0.f;
+        for (int t = 0; t < cnt; ++t) s = fmaf(w[(k0 + t) * ldw + c * (lmax + 1) + l], Ys[t][lm], s);
+        acc[q] += s;
+      }
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < MAXO; ++q) {
+    const int o = threadIdx.x + q * blockDim.x;
+    if (o < nout) gamma[a * nout + o] = inv_sqrt_navg * acc[q];
+  }
+}
+
+// B5 (row reduction) + B6: Gammabar_i = sum_row GE[e], then for every edge of the row
+//   wbar[e,c,l] = Nbar^-1/2 sum_m Gammabar[c,l,m] Y_lm(e);   Ybar[e,lm] += Nbar^-1/2 sum_c w[e,c,l] Gammabar[c,lm].
+// One block per centre atom, Gammabar kept in shared memory.
+__global__ void k_gammabar(const int64_t* __restrict__ rowptr_c, const float* __restrict__ geo, const float* __restrict__ ge,
+                           const float* __restrict__ w, int ldw, int n, int lmax, float inv_sqrt_navg,
+                           float* __restrict__ wbar, int ldwb, float* __restrict__ ybar, int64_t n_atoms) {
+  extern __shared__ float sm[];
+  const int64_t a = blockIdx.x;
+  if (a >= n_atoms) return;
+  const int dsh = (lmax + 1) * (lmax + 1), nout = n * dsh, nsc = n * (lmax + 1);
+  float* Gb = sm;              // [nout]
+  float* Ys = sm + nout;       // [16]
+  const int64_t b = rowptr_c[a], e = rowptr_c[a + 1];
+  for (int o = threadIdx.x; o < nout; o += blockDim.x) {
+    float s = 0.f;
+    for (int64_t k = b; k < e; ++k) s += ge[k * nout + o];
+    Gb[o] = s * inv_sqrt_navg;
+  }
+  for (int64_t k = b; k < e; ++k) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      const float* gq = geo + k * GEO_W;
+      sph_harm_rt(lmax, gq[0], gq[1], gq[2], Ys);
+    }
+    __syncthreads();
+    for (int o = threadIdx.x; o < nsc; o += blockDim.x) {
+      const int c = o / (lmax + 1), l = o - c * (lmax + 1);
+      float s = 0.f;
+      for (int mm = 0; mm < 2 * l + 1; ++mm) s = fmaf(Gb[c * dsh + l * l + mm], Ys[l * l + mm], s);
+      wbar[k * ldwb + o] = s;
+    }
+    if (threadIdx.x < dsh) {
+      const int lm = threadIdx.x;
+      const int l = (lm >= 9) ? 3 : (lm >= 4) ? 2 : (lm >= 1) ? 1 : 0;
+      float s = 0.f;
+      for (int c = 0; c < n; ++c) s = fmaf(w[k * ldw + c * (lmax + 1) + l], Gb[c * dsh + lm], s);
+      ybar[k * dsh + lm] += s;
+    }
+  }
+}
+
+// B8: wbar_init[e,c,l] = sum_m Vbar0[e,c,l,m] Y_lm;  Ybar[e,lm] += sum_c winit[e,c,l] Vbar0[e,c,lm].  One warp per edge.
+__global__ void k_init_bwd(const int64_t* __restrict__ Mptr, const float* __restrict__ geo, const float* __restrict__ vbar0,
+                           const float* __restrict__ winit, int ldwi, int n, int lmax, float* __restrict__ wbar, int ldwb,
+                           float* __restrict__ ybar) {
+  const int lane = threadIdx.x & 31;
+  const int64_t e = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (e >= *Mptr) return;
+  const int dsh = (lmax + 1) * (lmax + 1);
+  float Y[16], yb[16];
+  const float* gq = geo + e * GEO_W;
+  sph_harm_rt(lmax, gq[0], gq[1], gq[2], Y);
+#pragma unroll
+  for (int q = 0; q < 16; ++q) yb[q] = 0.f;
+  for (int c = lane; c < n; c += 32) {
+    const float* vb = vbar0 + (e * n + c) * dsh;
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+      if (l <= lmax) {
+        const float wi = winit[e * ldwi + c * (lmax + 1) + l];
+        float s = 0.f;
+#pragma unroll
+        for (int mm = 0; mm < 2 * l + 1; ++mm) {
+          const float v = vb[l * l + mm];
+          s = fmaf(v, Y[l * l + mm], s);
+          yb[l * l + mm] = fmaf(wi, v, yb[l * l + mm]);
+        }
+        wbar[e * ldwb + c * (lmax + 1) + l] = s;
+      }
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < 16; ++q) {
+    if (q < dsh) {
+      float v = yb[q];
+#pragma unroll
+      for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+      if (lane == 0) ybar[e * dsh + q] += v;
+    }
+  }
+}
+
+// B1: xbar^{NL}[e, :] = sigma_{Z_i} * w_eff  (the edge-energy chain has no non-linearity: PAPER.md:93)
+__global__ void k_xbar_init(const int64_t* __restrict__ Mptr, const float* __restrict__ geo, const float* __restrict__ sigma,
+                            const float* __restrict__ weff, int D, float* __restrict__ xbar) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t e = idx / D;
+  if (e >= *Mptr) return;
+  const int d = (int)(idx - e * D);
+  xbar[idx] = sigma[__float_as_int(geo[e * GEO_W + 6])] * weff[d];
+}
+
+// out[e] (+)= scale * dot(A[e,:], B[e,:])   (ubar contributions of B3 and B9).  One warp per edge.
+__global__ void k_rowdot(const int64_t* __restrict__ Mptr, const float* __restrict__ A, const float* __restrict__ B, int D,
+                         float scale, int accumulate, float* __restrict__ out) {
+  const int lane = threadIdx.x & 31;
+  const int64_t e = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (e >= *Mptr) return;
+  float s = 0.f;
+  for (int d = lane; d < D; d += 32) s = fmaf(A[e * D + d], B[e * D + d], s);
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+  if (lane == 0) out[e] = (accumulate ? out[e] : 0.f) + scale * s;
+}
+
+// F12: eps_e = w_eff . x^{NL}_e;  E_i = sigma_{Z_i} sum_row eps_e + mu_{Z_i}.  One warp per centre atom.
+__global__ void k_readout(const int64_t* __restrict__ rowptr_c, const float* __restrict__ x, int D, const float* __restrict__ weff,
+                          const int* __restrict__ species, int64_t a0, int64_t n_atoms, const float* __restrict__ sigma,
+                          const float* __restrict__ mu, float* __restrict__ e_atom) {
+  const int lane = threadIdx.x & 31;
+  const int64_t a = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (a >= n_atoms) return;
+  float s = 0.f;
+  for (int64_t k = rowptr_c[a]; k < rowptr_c[a + 1]; ++k)
+    for (int d = lane; d < D; d += 32) s = fmaf(x[k * D + d], weff[d], s);
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+  if (lane == 0) {
+    const int z = species[a0 + a];
+    e_atom[a0 + a] = sigma[z] * s + mu[z];
+  }
+}
+
+// B10 + B11: g_e = rbar rhat + (1/r)(I - rhat rhat^T) sum_lm Ybar_lm grad Y_lm, written at the edge's list position.
+__global__ void k_edge_grad(const int64_t* __restrict__ Mptr, const float* __restrict__ geo, const float* __restrict__ bes,
+                            const float* __restrict__ bbar, const float* __restrict__ ubar, const float* __restrict__ ybar,
+                            const int64_t* __restrict__ e_lidx, int n_bessel, int lmax, float rc, float* __restrict__ g_list) {
+  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= *Mptr) return;
+  const float* gq = geo + e * GEO_W;
+  const float x = gq[0], y = gq[1], z = gq[2], r = gq[3], u = gq[4], du = gq[5];
+  const int dsh = (lmax + 1) * (lmax + 1);
+  // d b_n/dr = (2/rc)(k cos(kr)/r - sin(kr)/r^2) u + B_n du  with B_n u = b_n  =>  = (2/rc) k cos(kr) u / r - b_n / r + (b_n/u) du
+  float rbar = ubar[e] * du;
+  const float inv_r = 1.0f / r, pref = 2.0f / rc;
+  for (int n = 1; n <= n_bessel; ++n) {
+    const float k = n * 3.14159265358979f / rc;
+    float sn, cs;
+    sincosf(k * r, &sn, &cs);
+    const float Bn = pref * sn * inv_r;
+    const float dBn = pref * (k * cs * inv_r - sn * inv_r * inv_r);
+    rbar = fmaf(bbar[e * n_bessel + (n - 1)], dBn * u + Bn * du, rbar);
+  }
+  float Yb[16], t[3];
+  for (int q = 0; q < dsh; ++q) Yb[q] = ybar[e * dsh + q];
+  sph_harm_vjp(lmax, x, y, z, Yb, t);
+  const float tr = t[0] * x + t[1] * y + t[2] * z;
+  const int64_t k = e_lidx[e];
+  g_list[3 * k] = rbar * x + (t[0] - tr * x) * inv_r;
+  g_list[3 * k + 1] = rbar * y + (t[1] - tr * y) * inv_r;
+  g_list[3 * k + 2] = rbar * z + (t[2] - tr * z) * inv_r;
+}
+
+// B12: F_i = sum_{e in row(i)} (g_e - g_rev(e)), accumulated in fp64 in CSR order.  One warp per atom.
+__global__ void k_force_gather(ListView lv, int64_t N, const float* __restrict__ g_list, double* __restrict__ F, int* flags) {
+  const int lane = threadIdx.x & 31;
+  const int64_t i = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (i >= N) return;
+  double fx = 0, fy = 0, fz = 0;
+  for (int64_t k = lv.rowptr[i] + lane; k < lv.rowptr[i + 1]; k += 32) {
+    const int j = (int)(lv.keys[k] >> 24);
+    const int64_t kr = lv.rowptr[j] + lv.revpos[k];
+    fx += (double)g_list[3 * k] - (double)g_list[3 * kr];
+    fy += (double)g_list[3 * k + 1] - (double)g_list[3 * kr + 1];
+    fz += (double)g_list[3 * k + 2] - (double)g_list[3 * kr + 2];
+  }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) {
+    fx += __shfl_xor_sync(0xffffffffu, fx, d);
+    fy += __shfl_xor_sync(0xffffffffu, fy, d);
+    fz += __shfl_xor_sync(0xffffffffu, fz, d);
+  }
+  if (lane == 0) {
+    F[3 * i] = fx; F[3 * i + 1] = fy; F[3 * i + 2] = fz;
+    if (!(isfinite(fx) && isfinite(fy) && isfinite(fz))) flags[FLAG_NONFINITE] = 1;
+  }
+}
+
+// E = sum_i E_i in fp64: fixed-shape two-stage tree (deterministic)
+__global__ void k_energy_partial(const float* __restrict__ e_atom, int64_t N, double* __restrict__ partial) {
+  __shared__ double sh[256];
+  double s = 0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (int64_t)gridDim.x * blockDim.x) s += (double)e_atom[i];
+  sh[threadIdx.x] = s;
+  __syncthreads();
+  for (int d = 128; d > 0; d >>= 1) {
+    if (threadIdx.x < d) sh[threadIdx.x] += sh[threadIdx.x + d];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) partial[blockIdx.x] = sh[0];
+}
+__global__ void k_energy_final(const double* __restrict__ partial, int nb, double* __restrict__ E, int* flags) {
+  __shared__ double sh[256];
+  double s = 0;
+  for (int i = threadIdx.x; i < nb; i += blockDim.x) s += partial[i];
+  sh[threadIdx.x] = s;
+  __syncthreads();
+  for (int d = 128; d > 0; d >>= 1) {
+    if (threadIdx.x < d) sh[threadIdx.x] += sh[threadIdx.x + d];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) { *E = sh[0]; if (!isfinite(sh[0])) flags[FLAG_NONFINITE] = 1; }
+}
+
+}  // namespace allegro

@@ -1,0 +1,111 @@
+// model.h — device-side state of one allegro handle and the launchers shared by the .cu files.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "plan.h"
+
+namespace allegro {
+
+// geometry record per active edge: 8 floats = two float4 (SoA of records keeps 128-bit loads)
+//   [0..2] unit vector rhat, [3] r, [4] u(r/rc), [5] du/dr, [6] bit-cast int zi, [7] bit-cast int zj
+constexpr int GEO_W = 8;
+
+struct DevBuf {
+  void* p = nullptr;
+  size_t bytes = 0;
+  template <class T> T* as() const { return reinterpret_cast<T*>(p); }
+};
+
+struct CgDev {           // one tensor-product layer's tables on the device
+  int n_paths = 0;
+  int* path_tab = nullptr;   // [n_paths][8]: in_off, d1, l2off, d2, out_irrep, pidx, cg_begin, cg_end
+  int* cg_idx = nullptr;     // [nnz] packed m1 | m2<<8 | m3<<16
+  float* cg_val = nullptr;   // [nnz]
+};
+
+struct NeighborList {
+  bool valid = false;
+  int64_t N = 0;
+  double L[3] = {0, 0, 0};
+  double cutoff = 0, skin = 0;
+  int nc[3] = {1, 1, 1};
+  int64_t E_list = 0, cap = 0;
+  int64_t n_rebuilds = 0;
+  DevBuf r_build, img, cell_of, cell_cnt, cell_start, cell_fill, sorted, row_cnt, rowptr, keys_tmp, keys, revpos;
+  DevBuf scan_tmp;
+};
+
+struct Workspace {       // per-chunk activations, sized for cap_edges active edges and cap_atoms atoms
+  int64_t cap_edges = 0, cap_atoms = 0;
+  DevBuf arena;          // one allocation, carved below
+  // chunk-local CSR of active edges
+  int* act_cnt = nullptr; int64_t* rowptr_c = nullptr; DevBuf scan_tmp;
+  int* e_center = nullptr; int* e_j = nullptr; int64_t* e_lidx = nullptr;
+  float* geo = nullptr; float* bes = nullptr;
+  std::vector<float*> z2b;           // two-body hidden pre-activations
+  float* y0 = nullptr;
+  std::vector<float*> x;             // x^0..x^NL
+  std::vector<float*> wenv;          // wenv[L-1]: [E, n_sc] (layer 1: second half of winit_w1)
+  float* winit_w1 = nullptr;         // [E, 2 n_sc] = W_init x0 | W_env^1 x0
+  std::vector<float*> s;             // scalars per layer
+  std::vector<std::vector<float*>> zlat;  // latent hidden pre-activations per layer
+  std::vector<float*> ylat;          // latent MLP outputs per layer
+  std::vector<float*> V;             // V^1..V^{NL-1}  ([E, n, out_dim])
+  std::vector<float*> gamma;         // per layer [atoms, n, d_sh]
+  // backward
+  float* xb[2] = {nullptr, nullptr}; float* zb[2] = {nullptr, nullptr};
+  float* sb = nullptr; float* vb[2] = {nullptr, nullptr}; float* ge = nullptr; float* wb = nullptr;
+  float* yb = nullptr; float* ub = nullptr; float* bb = nullptr; float* gammab = nullptr;
+};
+
+struct Model {
+  Plan plan;
+  std::string err;
+  int device = 0;
+  int num_sms = 148;
+  float* d_w = nullptr;            // weight blob
+  float* d_weff = nullptr;         // collapsed edge-energy chain W_last...W_1 -> [D]
+  std::vector<CgDev> cg;           // per layer
+  std::vector<float> c_old, c_new; // host copies
+  NeighborList nl;
+  Workspace ws;
+  // global per-list-edge gradient and per-atom outputs
+  DevBuf g_list, e_atom, e_partial, flags, md_pos, md_vel, md_mass, md_species, md_F, md_E;
+  bool md_ready = false;
+  double md_cell[9] = {0};
+  int64_t stats[8] = {0};
+  int64_t launches = 0;
+};
+
+// device flag slots (int32 array in Model::flags)
+enum { FLAG_REBUILD = 0, FLAG_ERR_SHIFT = 1, FLAG_ERR_CAP = 2, FLAG_STALE = 3, FLAG_NONFINITE = 4, FLAG_SPECIES = 5,
+       FLAG_NREBUILD = 6, FLAG_COUNT = 16 };
+
+// ---- helpers (api.cu)
+int ensure(Model* m, DevBuf* b, size_t bytes);            // grow-only cudaMalloc; 0 or ALLEGRO_ERR_ALLOC
+int cuda_fail(Model* m, cudaError_t e, const char* what);  // records message, returns ALLEGRO_ERR_CUDA
+
+// ---- scan.cu: exclusive scan of n int32 counts into n+1 int64 offsets (device), optionally conditional on *flag != 0
+int scan_counts(Model* m, const int* cnt, int64_t* out, int64_t n, DevBuf* tmp, const int* flag, cudaStream_t st);
+
+// ---- neighbor.cu
+int nl_build(Model* m, const double* pos, int64_t N, const double* cell, double cutoff, double skin,
+             bool conditional, cudaStream_t st);
+int nl_export(Model* m, int64_t* rowptr, int32_t* col, int8_t* shift, cudaStream_t st);
+
+// ---- network.cu
+int ws_prepare(Model* m, int64_t cap_edges, int64_t cap_atoms);
+int network_energy_forces(Model* m, const double* pos, const int32_t* species, int64_t N,
+                          double* E_out, double* F_out, float* E_atom_out, cudaStream_t st);
+
+// ---- md.cu
+int md_init(Model* m, const double* pos, const double* vel, const double* mass, const int32_t* species, int64_t N,
+            const double* cell, double cutoff, double skin, cudaStream_t st);
+int md_step(Model* m, double dt, int64_t n_steps, cudaStream_t st);
+int md_kinetic(Model* m, double* Ekin_dev, cudaStream_t st);
+
+}  // namespace allegro

@@ -1,0 +1,356 @@
+// network.cu — rows a-2..a-5: orchestration of one energy+force evaluation (forward F1-F12, analytic backward
+// B1-B12 of SURVEY.md 8c) over the active edges of the current neighbour list, in chunks of centre atoms
+// (exact: the model is strictly local).
+#include <algorithm>
+#include <cmath>
+
+#include "edge_kernels.cuh"
+#include "gemm.cuh"
+#include "model.h"
+#include "tp.cuh"
+
+namespace allegro {
+
+namespace {
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+}
+
+// bytes of workspace per active edge / per atom of a chunk
+static void ws_sizes(const Plan& P, size_t* per_edge, size_t* per_atom) {
+  const allegro_hparams& hp = P.hp;
+  const int n = hp.n_channels, NL = hp.n_layers;
+  size_t f = GEO_W + hp.n_bessel;
+  for (int i = 0; i + 1 < hp.two_body_nl; ++i) f += hp.two_body_dims[i];
+  f += P.D;                         // y0
+  f += (size_t)(NL + 1) * P.D;      // x^0..x^NL
+  f += 2 * P.n_sc;                  // winit | w1
+  int maxh = 4, maxv = 4;
+  for (int L = 1; L <= NL; ++L) {
+    const Layer& ly = P.layers[L - 1];
+    if (L >= 2) f += P.n_sc;        // w^L
+    f += P.n_sc;                    // s^L
+    for (int i = 0; i + 1 < hp.latent_nl; ++i) { f += hp.latent_dims[i]; maxh = std::max(maxh, hp.latent_dims[i]); }
+    f += P.D;                       // y^L
+    if (L < NL) f += (size_t)n * ly.out_dim;
+    maxv = std::max(maxv, std::max(ly.in_dim, ly.out_dim));
+  }
+  for (int i = 0; i + 1 < hp.two_body_nl; ++i) maxh = std::max(maxh, hp.two_body_dims[i]);
+  f += 2 * P.D + 2 * maxh + P.n_sc + 2 * (size_t)n * maxv + (size_t)n * P.d_sh + 2 * P.n_sc + P.d_sh + 1 + hp.n_bessel;
+  *per_edge = f * sizeof(float) + 2 * sizeof(int) + sizeof(int64_t) + 64;
+  *per_atom = ((size_t)NL + 1) * n * P.d_sh * sizeof(float) + sizeof(int) + sizeof(int64_t) + 64;
+}
+
+int ws_prepare(Model* m, int64_t cap_edges, int64_t cap_atoms) {
+  Workspace& ws = m->ws;
+  if (cap_edges <= ws.cap_edges && cap_atoms <= ws.cap_atoms && ws.arena.p) return 0;
+  cap_edges = std::max<int64_t>(cap_edges, 256);
+  cap_atoms = std::max<int64_t>(cap_atoms, 32);
+  const Plan& P = m->plan;
+  const allegro_hparams& hp = P.hp;
+  const int n = hp.n_channels, NL = hp.n_layers;
+  size_t pe, pa;
+  ws_sizes(P, &pe, &pa);
+  const size_t total = pe * cap_edges + pa * (cap_atoms + 1) + (1 << 16);
+  if (int rc = ensure(m, &ws.arena, total)) return rc;
+  char* base = ws.arena.as<char>();
+  size_t off = 0;
+  auto carve = [&](size_t bytes) { void* p = base + off; off = align_up(off + bytes, 256); return p; };
+  auto cf = [&](size_t count) { return (float*)carve(count * sizeof(float)); };
+  const size_t E = (size_t)cap_edges, A = (size_t)cap_atoms;
+  ws.act_cnt = (int*)carve((A + 1) * sizeof(int));
+  ws.rowptr_c = (int64_t*)carve((A + 2) * sizeof(int64_t));
+  ws.e_center = (int*)carve(E * sizeof(int));
+  ws.e_j = (int*)carve(E * sizeof(int));
+  ws.e_lidx = (int64_t*)carve(E * sizeof(int64_t));
+  ws.geo = cf(E * GEO_W);
+  ws.bes = cf(E * hp.n_bessel);
+  ws.z2b.clear();
+  for (int i = 0; i + 1 < hp.two_body_nl; ++i) ws.z2b.push_back(cf(E * hp.two_body_dims[i]));
+  ws.y0 = cf(E * P.D);
+  ws.x.clear();
+  for (int L = 0; L <= NL; ++L) ws.x.push_back(cf(E * P.D));
+  ws.winit_w1 = cf(E * 2 * P.n_sc);
+  ws.wenv.assign(NL, nullptr); ws.s.clear(); ws.zlat.assign(NL, {}); ws.ylat.clear(); ws.V.assign(NL, nullptr); ws.gamma.clear();
+  int maxh = 4, maxv = 4;
+  for (int i = 0; i + 1 < hp.two_body_nl; ++i) maxh = std::max(maxh, hp.two_body_dims[i]);
+  for (int L = 1; L <= NL; ++L) {
+    const Layer& ly = P.layers[L - 1];
+    ws.wenv[L - 1] = (L == 1) ? ws.winit_w1 + P.n_sc : cf(E * P.n_sc);
+    ws.s.push_back(cf(E * P.n_sc));
+    for (int i = 0; i + 1 < hp.latent_nl; ++i) { ws.zlat[L - 1].push_back(cf(E * hp.latent_dims[i])); maxh = std::max(maxh, hp.latent_dims[i]); }
+    ws.ylat.push_back(cf(E * P.D));
+    if (L < NL) ws.V[L - 1] = cf(E * n * ly.out_dim);
+    ws.gamma.push_back(cf(A * n * P.d_sh));
+    maxv = std::max(maxv, std::max(ly.in_dim, ly.out_dim));
+  }
+  ws.xb[0] = cf(E * P.D); ws.xb[1] = cf(E * P.D);
+  ws.zb[0] = cf(E * maxh); ws.zb[1] = cf(E * maxh);
+  ws.sb = cf(E * P.n_sc);
+  ws.vb[0] = cf(E * n * maxv); ws.vb[1] = cf(E * n * maxv);
+  ws.ge = cf(E * n * P.d_sh);
+  ws.wb = cf(E * 2 * P.n_sc);
+  ws.yb = cf(E * P.d_sh);
+  ws.ub = cf(E);
+  ws.bb = cf(E * hp.n_bessel);
+  ws.gammab = cf(A * n * P.d_sh);
+  if (off > total) { m->err = "internal: workspace carve overflow"; return ALLEGRO_ERR_ALLOC; }
+  ws.cap_edges = cap_edges; ws.cap_atoms = cap_atoms;
+  return 0;
+}
+
+static TpLayerDev make_tp(const Model* m, int L) {
+  const Plan& P = m->plan;
+  const Layer& ly = P.layers[L - 1];
+  TpLayerDev t{};
+  t.n = P.hp.n_channels; t.lmax = P.hp.lmax; t.dsh = P.d_sh; t.in_dim = ly.in_dim; t.out_dim = ly.out_dim;
+  t.n_paths = (int)ly.paths.size(); t.n_out = (int)ly.out_irreps.size(); t.layer1 = (L == 1); t.has_lin = (L < P.hp.n_layers);
+  t.path_tab = m->cg[L - 1].path_tab; t.cg_idx = m->cg[L - 1].cg_idx; t.cg_val = m->cg[L - 1].cg_val;
+  for (int o = 0; o < t.n_out; ++o) {
+    t.out_d3[o] = 2 * ly.out_irreps[o].l + 1; t.out_off[o] = ly.out_off[o]; t.out_np[o] = ly.out_npaths[o];
+    t.wlin[o] = ly.w_lin[o];
+  }
+  return t;
+}
+
+// forward + backward for the centre atoms [a0, a1); m_cap bounds the number of active edges (list edges of the chunk)
+static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_t a0, int64_t a1, int64_t m_cap, cudaStream_t st) {
+  const Plan& P = m->plan;
+  const allegro_hparams& hp = P.hp;
+  Workspace& ws = m->ws;
+  NeighborList& nl = m->nl;
+  int* flags = m->flags.as<int>();
+  const int n = hp.n_channels, NL = hp.n_layers, D = P.D, nsc = P.n_sc, dsh = P.d_sh, S = hp.n_species, Nb = hp.n_bessel;
+  const int64_t na = a1 - a0;
+  const float inv_sqrt_navg = (float)(1.0 / std::sqrt(hp.avg_num_neighbors));
+  ListView lv{nl.rowptr.as<int64_t>(), nl.keys.as<uint64_t>(), nl.revpos.as<int>(), {nl.L[0], nl.L[1], nl.L[2]}};
+  const int T = 256;
+  const unsigned gridWA = (unsigned)((na * 32 + T - 1) / T);
+  // ---- active edges of the chunk
+  k_active<0><<<gridWA, T, 0, st>>>(pos, species, lv, a0, a1, hp.r_cut, hp.poly_p, Nb, ws.act_cnt, nullptr, nullptr, nullptr, nullptr,
+                                    nullptr, nullptr, nullptr, 0, flags);
+  if (int rc = scan_counts(m, ws.act_cnt, ws.rowptr_c, na, &ws.scan_tmp, nullptr, st)) return rc;
+  k_active<1><<<gridWA, T, 0, st>>>(pos, species, lv, a0, a1, hp.r_cut, hp.poly_p, Nb, nullptr, ws.rowptr_c, ws.e_center, ws.e_j,
+                                    ws.e_lidx, ws.geo, ws.bes, m->g_list.as<float>(), ws.cap_edges, flags);
+  m->launches += 2;
+  const int64_t* Mptr = ws.rowptr_c + na;
+  const float* w = m->d_w;
+  const unsigned gridE = (unsigned)((m_cap + T - 1) / T), gridWE = (unsigned)((m_cap * 32 + T - 1) / T);
+  if (m_cap <= 0) return 0;
+
+  // ---- F4: two-body MLP.  First layer = gather of the two one-hot columns + N_b-wide mat-vec.
+  GemmArgs g;
+  const int fan0 = 2 * S + Nb;
+  {
+    g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo;
+    g.A0 = ws.bes; g.lda0 = Nb; g.K0 = Nb;
+    g.W = w + P.w_two_body[0] + 2 * S; g.ldw = fan0; g.wtrans = 0; g.N = hp.two_body_dims[0];
+    g.Wg = w + P.w_two_body[0]; g.ldwg = fan0; g.S = S; g.epi = EPI_GATHER2;
+    if (hp.two_body_nl == 1) { m->err = "two_body MLP needs at least 2 linear layers"; return ALLEGRO_ERR_UNSUPPORTED; }
+    g.C = ws.z2b[0]; g.ldc = hp.two_body_dims[0];
+    launch_gemm(m, g, m_cap, st);
+    for (int i = 1; i < hp.two_body_nl; ++i) {
+      g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo;
+      g.A0 = ws.z2b[i - 1]; g.lda0 = g.K0 = hp.two_body_dims[i - 1]; g.pro = PRO_SILU;
+      g.W = w + P.w_two_body[i]; g.ldw = hp.two_body_dims[i - 1]; g.N = hp.two_body_dims[i];
+      if (i + 1 < hp.two_body_nl) { g.C = ws.z2b[i]; g.ldc = g.N; g.epi = EPI_STORE; }
+      else { g.C = ws.y0; g.ldc = D; g.C2 = ws.x[0]; g.ldc2 = D; g.epi = EPI_Y_X; }   // x0 = u * y0
+      launch_gemm(m, g, m_cap, st);
+    }
+  }
+  // ---- F5/F6 (layer 1): [W_init; W_env^1] x0 in one GEMM (adjacent in the blob)
+  g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo;
+  g.A0 = ws.x[0]; g.lda0 = g.K0 = D; g.W = w + P.w_init; g.ldw = D; g.N = 2 * nsc; g.C = ws.winit_w1; g.ldc = 2 * nsc;
+  launch_gemm(m, g, m_cap, st);
+
+  std::vector<TpLayerDev> tps;
+  std::vector<int> te_f(NL), te_b(NL), d3m(NL);
+  for (int L = 1; L <= NL; ++L) {
+    const Layer& ly = P.layers[L - 1];
+    tps.push_back(make_tp(m, L));
+    const TpLayerDev& tp = tps.back();
+    const int ldw_env = (L == 1) ? 2 * nsc : nsc;
+    if (L >= 2) {   // F6
+      g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo;
+      g.A0 = ws.x[L - 1]; g.lda0 = g.K0 = D; g.W = w + ly.w_env; g.ldw = D; g.N = nsc; g.C = ws.wenv[L - 1]; g.ldc = nsc;
+      launch_gemm(m, g, m_cap, st);
+    }
+    // F7
+    k_gamma<<<(unsigned)na, 128, 0, st>>>(ws.rowptr_c, ws.geo, ws.wenv[L - 1], ldw_env, n, hp.lmax, inv_sqrt_navg, ws.gamma[L - 1], na);
+    // F8, F9, F11
+    int d3max = 1;
+    for (int o = 0; o < tp.n_out; ++o) if (tp.has_lin || o == 0) d3max = std::max(d3max, tp.out_d3[o]);
+    d3m[L - 1] = d3max;
+    int TE = (16 * TP_T * TP_MAXMT) / (n * d3max);
+    TE = std::max(4, std::min(64, TE / 4 * 4));
+    while ((size_t)(n * TE * d3max + n * n + TE * 16) * sizeof(float) > 200 * 1024 && TE > 4) TE -= 4;
+    te_f[L - 1] = TE;
+    TpIo io{}; io.Mptr = Mptr; io.e_center = ws.e_center; io.geo = ws.geo; io.gamma = ws.gamma[L - 1];
+    io.vprev = (L >= 2) ? ws.V[L - 2] : nullptr; io.winit = ws.winit_w1; io.ldwi = 2 * nsc; io.w = w;
+    io.s = ws.s[L - 1]; io.vout = (L < NL) ? ws.V[L - 1] : nullptr;
+    {
+      size_t smem = (size_t)(n * TE * d3max + n * n + TE * 16) * sizeof(float);
+      cudaFuncSetAttribute(k_tp_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      dim3 grid((unsigned)((m_cap + TE - 1) / TE), (unsigned)(tp.has_lin ? tp.n_out : 1));
+      k_tp_fwd<<<grid, TP_T, smem, st>>>(tp, io, TE);
+    }
+    m->launches += 2;
+    // F10: latent MLP on (x | s), residual update
+    for (int i = 0; i < hp.latent_nl; ++i) {
+      g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo;
+      if (i == 0) { g.A0 = ws.x[L - 1]; g.lda0 = g.K0 = D; g.A1 = ws.s[L - 1]; g.lda1 = g.K1 = nsc; g.ldw = D + nsc; }
+      else { g.A0 = ws.zlat[L - 1][i - 1]; g.lda0 = g.K0 = hp.latent_dims[i - 1]; g.pro = PRO_SILU; g.ldw = hp.latent_dims[i - 1]; }
+      g.W = w + ly.w_latent[i]; g.N = hp.latent_dims[i];
+      if (i + 1 < hp.latent_nl) { g.C = ws.zlat[L - 1][i]; g.ldc = g.N; }
+      else {
+        g.C = ws.ylat[L - 1]; g.ldc = D; g.C2 = ws.x[L]; g.ldc2 = D; g.aux = ws.x[L - 1]; g.ldaux = D;
+        g.c_old = m->c_old[L - 1]; g.c_new = m->c_new[L - 1]; g.epi = EPI_RESIDUAL;
+        if (hp.latent_nl == 1) { m->err = "latent MLP needs at least 2 linear layers"; return ALLEGRO_ERR_UNSUPPORTED; }
+      }
+      launch_gemm(m, g, m_cap, st);
+    }
+  }
+  // ---- F12
+  k_readout<<<gridWA, T, 0, st>>>(ws.rowptr_c, ws.x[NL], D, m->d_weff, species, a0, na, w + P.w_sigma, w + P.w_mu, m->e_atom.as<float>());
+  m->launches += 1;
+
+  // ================= backward =================
+  cudaMemsetAsync(ws.yb, 0, sizeof(float) * (size_t)m_cap * dsh, st);
+  k_xbar_init<<<(unsigned)((m_cap * D + T - 1) / T), T, 0, st>>>(Mptr, ws.geo, w + P.w_sigma, m->d_weff, D, ws.xb[0]);   // B1
+  m->launches += 1;
+  int xcur = 0, vcur = 0;
+  bool ub_init = false;
+  for (int L = NL; L >= 1; --L) {
+    const Layer& ly = P.layers[L - 1];
+    const TpLayerDev& tp = tps[L - 1];
+    const float c_old = m->c_old[L - 1], c_new = m->c_new[L - 1];
+    // B3: ubar += c_new (xbar . y)
+    k_rowdot<<<gridWE, T, 0, st>>>(Mptr, ws.xb[xcur], ws.ylat[L - 1], D, c_new, ub_init ? 1 : 0, ws.ub);
+    ub_init = true;
+    m->launches += 1;
+    // B3/B4: latent MLP backward.  ybar = c_new u xbar is applied as the prologue of the first transposed GEMM.
+    {
+      const float* cur = ws.xb[xcur];
+      int zc = 0;
+      for (int i = hp.latent_nl - 1; i >= 0; --i) {
+        const int in_w = (i == 0) ? D + nsc : hp.latent_dims[i - 1];
+        g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo; g.wtrans = 1;
+        g.W = w + ly.w_latent[i]; g.ldw = in_w; g.N = in_w;
+        g.A0 = cur; g.lda0 = g.K0 = hp.latent_dims[i];
+        if (i == hp.latent_nl - 1) { g.pro = PRO_SCALE_U; g.c_new = c_new; }
+        if (i > 0) {   // zbar = hbar * silu'(z)
+          g.C = ws.zb[zc]; g.ldc = in_w; g.aux = ws.zlat[L - 1][i - 1]; g.ldaux = in_w; g.epi = EPI_DSILU;
+          cur = ws.zb[zc]; zc ^= 1;
+        } else {       // (xbar_in | sbar): xbar^{L-1} = c_old xbar^L + xbar_in
+          g.C = ws.xb[xcur ^ 1]; g.ldc = D; g.aux = ws.xb[xcur]; g.ldaux = D; g.c_old = c_old; g.split = D;
+          g.C2 = ws.sb; g.ldc2 = nsc; g.epi = EPI_SPLIT_RES;
+        }
+        launch_gemm(m, g, m_cap, st);
+      }
+    }
+    xcur ^= 1;
+    // B2 + B5: tensor-product backward -> Vbar^{L-1}, GE
+    {
+      const int d3max = d3m[L - 1];
+      const size_t per_edge = (size_t)n * (ly.in_dim + dsh) + 16;
+      int TE = 32;
+      auto smem_of = [&](int te) { return (per_edge * te + 2 * (size_t)n * te * d3max + (size_t)n * n) * sizeof(float); };
+      while (TE > 4 && smem_of(TE) > 200 * 1024) TE -= 4;
+      if (smem_of(TE) > 227 * 1024) { m->err = "tensor-product backward tile does not fit in shared memory"; return ALLEGRO_ERR_UNSUPPORTED; }
+      TpIo io{}; io.Mptr = Mptr; io.e_center = ws.e_center; io.geo = ws.geo; io.gamma = ws.gamma[L - 1];
+      io.vprev = (L >= 2) ? ws.V[L - 2] : nullptr; io.winit = ws.winit_w1; io.ldwi = 2 * nsc; io.w = w;
+      io.sbar = ws.sb; io.vbar = (L < NL) ? ws.vb[vcur] : nullptr; io.vbar_prev = ws.vb[vcur ^ 1]; io.ge = ws.ge;
+      size_t smem = smem_of(TE);
+      cudaFuncSetAttribute(k_tp_bwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      k_tp_bwd<<<(unsigned)((m_cap + TE - 1) / TE), TP_T, smem, st>>>(tp, io, TE, d3max);
+      vcur ^= 1;
+      m->launches += 1;
+    }
+    // B5 (row reduction) + B6
+    const int ldw_env = (L == 1) ? 2 * nsc : nsc;
+    float* wbar = (L == 1) ? ws.wb + nsc : ws.wb;
+    const int ldwb = (L == 1) ? 2 * nsc : nsc;
+    k_gammabar<<<(unsigned)na, 128, (size_t)(n * dsh + 16) * sizeof(float), st>>>(ws.rowptr_c, ws.geo, ws.ge, ws.wenv[L - 1], ldw_env, n,
+                                                                                  hp.lmax, inv_sqrt_navg, wbar, ldwb, ws.yb, na);
+    m->launches += 1;
+    if (L >= 2) {   // B7: xbar^{L-1} += W_env^T wbar
+      g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo; g.wtrans = 1;
+      g.A0 = ws.wb; g.lda0 = g.K0 = nsc; g.W = w + ly.w_env; g.ldw = D; g.N = D; g.C = ws.xb[xcur]; g.ldc = D; g.epi = EPI_ACCUM;
+      launch_gemm(m, g, m_cap, st);
+    }
+  }
+  // B8: adjoint of V^0, then [W_init; W_env^1]^T [wbar_init; wbar^1] in one GEMM (B7 of layer 1 + B8)
+  k_init_bwd<<<gridWE, T, 0, st>>>(Mptr, ws.geo, ws.vb[vcur], ws.winit_w1, 2 * nsc, n, hp.lmax, ws.wb, 2 * nsc, ws.yb);
+  g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo; g.wtrans = 1;
+  g.A0 = ws.wb; g.lda0 = g.K0 = 2 * nsc; g.W = w + P.w_init; g.ldw = D; g.N = D; g.C = ws.xb[xcur]; g.ldc = D; g.epi = EPI_ACCUM;
+  launch_gemm(m, g, m_cap, st);
+  // B9: ubar += xbar0 . y0;  two-body MLP backward with ybar0 = u xbar0
+  k_rowdot<<<gridWE, T, 0, st>>>(Mptr, ws.xb[xcur], ws.y0, D, 1.0f, 1, ws.ub);
+  m->launches += 2;
+  {
+    const float* cur = ws.xb[xcur];
+    int zc = 0;
+    for (int i = hp.two_body_nl - 1; i >= 1; --i) {
+      g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo; g.wtrans = 1;
+      g.W = w + P.w_two_body[i]; g.ldw = hp.two_body_dims[i - 1]; g.N = hp.two_body_dims[i - 1];
+      g.A0 = cur; g.lda0 = g.K0 = hp.two_body_dims[i];
+      if (i == hp.two_body_nl - 1) { g.pro = PRO_SCALE_U; g.c_new = 1.0f; }
+      g.C = ws.zb[zc]; g.ldc = g.N; g.aux = ws.z2b[i - 1]; g.ldaux = g.N; g.epi = EPI_DSILU;
+      cur = ws.zb[zc]; zc ^= 1;
+      launch_gemm(m, g, m_cap, st);
+    }
+    // bbar = W_1[:, 2S:]^T zbar_1
+    g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo; g.wtrans = 1;
+    g.A0 = cur; g.lda0 = g.K0 = hp.two_body_dims[0]; g.W = w + P.w_two_body[0] + 2 * S; g.ldw = fan0; g.N = Nb;
+    g.C = ws.bb; g.ldc = Nb;
+    launch_gemm(m, g, m_cap, st);
+  }
+  // B10, B11
+  k_edge_grad<<<gridE, T, 0, st>>>(Mptr, ws.geo, ws.bes, ws.bb, ws.ub, ws.yb, ws.e_lidx, Nb, hp.lmax, (float)hp.r_cut, m->g_list.as<float>());
+  m->launches += 1;
+  return 0;
+}
+
+int network_energy_forces(Model* m, const double* pos, const int32_t* species, int64_t N, double* E_out, double* F_out,
+                          float* E_atom_out, cudaStream_t st) {
+  NeighborList& nl = m->nl;
+  int* flags = m->flags.as<int>();
+  if (int rc = ensure(m, &m->e_atom, sizeof(float) * (N + 1))) return rc;
+  if (int rc = ensure(m, &m->e_partial, sizeof(double) * 1024)) return rc;
+  const int T = 256;
+  if (N > 0) {
+    const double hs = 0.5 * nl.skin;
+    k_check_inputs<<<(unsigned)((N + T - 1) / T), T, 0, st>>>(pos, nl.r_build.as<double>(), species, N, hs * hs, m->plan.hp.n_species, flags);
+    m->launches += 1;
+  }
+  // single chunk when the workspace fits; otherwise atom chunks bounded by list edges (sized with the average row)
+  size_t pe, pa;
+  ws_sizes(m->plan, &pe, &pa);
+  size_t free_b = 0, total_b = 0;
+  cudaMemGetInfo(&free_b, &total_b);
+  const size_t budget = (size_t)(0.80 * (double)(free_b + m->ws.arena.bytes));
+  int64_t n_chunks = 1;
+  const int64_t Ecap = std::max<int64_t>(nl.cap, 1);
+  while ((pe * (size_t)(Ecap / n_chunks + 1) * 1.25 + pa * (size_t)(N / n_chunks + 1)) > budget && n_chunks < N) n_chunks *= 2;
+  const int64_t atoms_per = (N + n_chunks - 1) / std::max<int64_t>(n_chunks, 1);
+  const int64_t edges_per = (n_chunks == 1) ? Ecap : (int64_t)((double)Ecap / n_chunks * 1.25) + 4096;
+  if (int rc = ws_prepare(m, edges_per, atoms_per)) return rc;
+  for (int64_t a0 = 0; a0 < N; a0 += atoms_per) {
+    const int64_t a1 = std::min(N, a0 + atoms_per);
+    if (int rc = run_chunk(m, pos, species, a0, a1, m->ws.cap_edges, st)) return rc;
+  }
+  ListView lv{nl.rowptr.as<int64_t>(), nl.keys.as<uint64_t>(), nl.revpos.as<int>(), {nl.L[0], nl.L[1], nl.L[2]}};
+  if (N > 0) {
+    k_force_gather<<<(unsigned)((N * 32 + T - 1) / T), T, 0, st>>>(lv, N, m->g_list.as<float>(), F_out, flags);
+    const int nb = (int)std::min<int64_t>(1024, (N + 255) / 256);
+    k_energy_partial<<<nb, 256, 0, st>>>(m->e_atom.as<float>(), N, m->e_partial.as<double>());
+    k_energy_final<<<1, 256, 0, st>>>(m->e_partial.as<double>(), nb, E_out, flags);
+    m->launches += 3;
+  } else {
+    cudaMemsetAsync(E_out, 0, sizeof(double), st);
+  }
+  if (E_atom_out && N > 0) cudaMemcpyAsync(E_atom_out, m->e_atom.p, sizeof(float) * N, cudaMemcpyDeviceToDevice, st);
+  m->stats[1] = nl.E_list;
+  return 0;
+}
+
+}  // namespace allegro
