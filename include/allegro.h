@@ -110,6 +110,15 @@ int allegro_get_neighbors(void* h, int64_t* rowptr, int32_t* col, int8_t* shift,
  * [4] force evaluations of the call, [5..7] reserved. */
 int allegro_get_stats(void* h, int64_t* stats);
 
+/* Per-kernel-class timing for bench.py's roofline line.  allegro_profile(h, 1) resets the counters and makes
+ * every launch of the following calls bracketed by CUDA events on the launching stream; allegro_profile(h, 0)
+ * stops it.  allegro_get_profile synchronises and returns, per class k (0 gemm, 1 tp_fwd, 2 tp_bwd, 3 gamma,
+ * 4 gammabar, 5 active_edges, 6 edge_misc, 7 neighbor, 8 md, 9 force_gather): ms[k] total device time,
+ * launches[k], work[k] = algorithmic flop per active edge summed over the class's launches (classes 0-2, else 0).
+ * HOST arrays of max_classes entries; returns the number of classes.  Never enabled inside a timed throughput run. */
+int allegro_profile(void* h, int enable);
+int allegro_get_profile(void* h, double* ms, int64_t* launches, double* work, int max_classes);
+
 /* Debug taps for the CPU-only tests (pure host logic, no CUDA): the library's own real coupling tensor
  * C^(l1 l2 l3) (reading A9), dense row-major [2l1+1][2l2+1][2l3+1] into out (HOST, fp64); and the number of
  * tensor-product paths of layer L (1-based) of the plan derived from hp.  Negative return = error. */

@@ -24,8 +24,10 @@ ERR_NAMES = {0: "OK", -1: "INVALID", -2: "UNSUPPORTED", -3: "CUDA", -4: "STALE_L
              -7: "SPECIES", -8: "NO_LIST", -9: "ALLOC"}
 EXPORTS = ["allegro_weight_layout", "allegro_create", "allegro_destroy", "allegro_build_neighbors",
            "allegro_energy_forces", "allegro_md_init", "allegro_md_step", "allegro_get_state",
-           "allegro_get_neighbors", "allegro_get_stats", "allegro_debug_coupling", "allegro_debug_num_paths",
-           "allegro_last_error"]
+           "allegro_get_neighbors", "allegro_get_stats", "allegro_profile", "allegro_get_profile",
+           "allegro_debug_coupling", "allegro_debug_num_paths", "allegro_last_error"]
+PROFILE_CLASSES = ["gemm", "tp_fwd", "tp_bwd", "gamma", "gammabar", "active_edges", "edge_misc", "neighbor", "md",
+                   "force_gather"]
 
 
 class HParams(C.Structure):
@@ -54,6 +56,8 @@ _lib.allegro_md_step.argtypes = [_vp, _dbl, _i64, _vp]
 _lib.allegro_get_state.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.allegro_get_neighbors.argtypes = [_vp, _vp, _vp, _vp, _vp]
 _lib.allegro_get_stats.argtypes = [_vp, _vp]
+_lib.allegro_profile.argtypes = [_vp, C.c_int]
+_lib.allegro_get_profile.argtypes = [_vp, _vp, _vp, _vp, C.c_int]
 _lib.allegro_debug_coupling.argtypes = [C.c_int, C.c_int, C.c_int, _vp]
 _lib.allegro_debug_num_paths.argtypes = [C.POINTER(HParams), C.c_int]
 _lib.allegro_last_error.argtypes = [_vp]
@@ -191,6 +195,16 @@ class Allegro:
         self._check(_lib.allegro_get_stats(self._h, s.ctypes.data))
         return dict(active_edges=int(s[0]), list_edges=int(s[1]), launches=int(s[2]), rebuilds=int(s[3]),
                     force_evals=int(s[4]))
+
+    def profile(self, enable: bool):
+        self._check(_lib.allegro_profile(self._h, 1 if enable else 0))
+
+    def get_profile(self) -> dict:
+        ms = np.zeros(16); ln = np.zeros(16, np.int64); wk = np.zeros(16)
+        n = _lib.allegro_get_profile(self._h, ms.ctypes.data, ln.ctypes.data, wk.ctypes.data, 16)
+        if n < 0:
+            self._check(n)
+        return {PROFILE_CLASSES[k]: dict(ms=float(ms[k]), launches=int(ln[k]), work=float(wk[k])) for k in range(n)}
 
     # convenience wrappers (allocation + marshalling only) ---------------------------------------
     def compute(self, pos_np, species_np, cell, skin=0.0, want_atom=False):

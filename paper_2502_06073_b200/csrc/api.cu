@@ -29,6 +29,33 @@ int cuda_fail(Model* m, cudaError_t e, const char* what) {
   return ALLEGRO_ERR_CUDA;
 }
 
+void prof_begin(Model* m, cudaStream_t st, int cls, double work) {
+  Prof& p = m->prof;
+  if (!p.on) return;
+  if (2 * p.used + 2 > p.ev.size()) {
+    for (int k = 0; k < 2; ++k) { cudaEvent_t e; cudaEventCreate(&e); p.ev.push_back(e); }
+    p.cls.push_back(cls);
+  }
+  p.cls[p.used] = cls;
+  p.work[cls] += work;
+  p.launches[cls] += 1;
+  cudaEventRecord(p.ev[2 * p.used], st);
+}
+void prof_end(Model* m, cudaStream_t st) {
+  Prof& p = m->prof;
+  if (!p.on) return;
+  cudaEventRecord(p.ev[2 * p.used + 1], st);
+  p.used += 1;
+}
+static void prof_collect(Model* m) {
+  Prof& p = m->prof;
+  for (size_t k = 0; k < p.used; ++k) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, p.ev[2 * k], p.ev[2 * k + 1]) == cudaSuccess) p.ms[p.cls[k]] += ms;
+  }
+  p.used = 0;
+}
+
 static void free_buf(DevBuf& b) { if (b.p) cudaFree(b.p); b.p = nullptr; b.bytes = 0; }
 
 static int check_flags(Model* m, cudaStream_t st, const char* what) {
@@ -173,6 +200,7 @@ int allegro_destroy(void* h) {
   Model* m = static_cast<Model*>(h);
   if (m->d_w) cudaFree(m->d_w);
   if (m->d_weff) cudaFree(m->d_weff);
+  for (cudaEvent_t e : m->prof.ev) cudaEventDestroy(e);
   for (CgDev& c : m->cg) { if (c.path_tab) cudaFree(c.path_tab); if (c.cg_idx) cudaFree(c.cg_idx); if (c.cg_val) cudaFree(c.cg_val); }
   NeighborList& nl = m->nl;
   for (DevBuf* b : {&nl.r_build, &nl.img, &nl.cell_of, &nl.cell_cnt, &nl.cell_start, &nl.cell_fill, &nl.sorted, &nl.row_cnt, &nl.rowptr,
@@ -295,6 +323,29 @@ int allegro_get_stats(void* h, int64_t* stats) {
   Model* m = static_cast<Model*>(h);
   for (int k = 0; k < 8; ++k) stats[k] = m->stats[k];
   return ALLEGRO_OK;
+}
+
+int allegro_profile(void* h, int enable) {
+  if (!h) return ALLEGRO_ERR_INVALID;
+  Model* m = static_cast<Model*>(h);
+  cudaDeviceSynchronize();
+  prof_collect(m);
+  m->prof.on = enable != 0;
+  if (enable) for (int k = 0; k < KC_COUNT; ++k) { m->prof.ms[k] = 0; m->prof.launches[k] = 0; m->prof.work[k] = 0; }
+  return ALLEGRO_OK;
+}
+
+int allegro_get_profile(void* h, double* ms, int64_t* launches, double* work, int max_classes) {
+  if (!h) return ALLEGRO_ERR_INVALID;
+  Model* m = static_cast<Model*>(h);
+  cudaDeviceSynchronize();
+  prof_collect(m);
+  for (int k = 0; k < KC_COUNT && k < max_classes; ++k) {
+    if (ms) ms[k] = m->prof.ms[k];
+    if (launches) launches[k] = m->prof.launches[k];
+    if (work) work[k] = m->prof.work[k];
+  }
+  return KC_COUNT;
 }
 
 const char* allegro_last_error(void* h) {

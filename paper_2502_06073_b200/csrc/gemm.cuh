@@ -155,7 +155,9 @@ __global__ void __launch_bounds__(GT) k_gemm(GemmArgs a) {
 inline void launch_gemm(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st) {
   if (m_cap <= 0) return;
   dim3 grid((unsigned)((m_cap + GM - 1) / GM), (unsigned)((a.N + GN - 1) / GN));
+  prof_begin(m, st, KC_GEMM, 2.0 * a.N * (a.K0 + a.K1));
   k_gemm<<<grid, GT, 0, st>>>(a);
+  prof_end(m, st);
   m->launches += 1;
 }
 

@@ -96,13 +96,19 @@ int md_step(Model* m, double dt, int64_t n_steps, cudaStream_t st) {
   const unsigned g3 = (unsigned)((3 * N + T - 1) / T), g1 = (unsigned)((N + T - 1) / T);
   const double hs = 0.5 * nl.skin;
   for (int64_t s = 0; s < n_steps; ++s) {
+    prof_begin(m, st, KC_MD, 0);
     k_kick_drift<<<g3, T, 0, st>>>(pos, vel, F, m->md_mass.as<double>(), N, dt, 1);
     k_skin_test<<<g1, T, 0, st>>>(pos, nl.r_build.as<double>(), N, hs * hs, nl.skin == 0.0 ? 1 : 0, flags);
+    prof_end(m, st);
     m->launches += 2;
+    prof_begin(m, st, KC_NEIGHBOR, 0);
     if (int rc = nl_build(m, pos, N, m->md_cell, nl.cutoff, nl.skin, true, st)) return rc;
     k_clear_flag<<<1, 1, 0, st>>>(flags, FLAG_REBUILD);
+    prof_end(m, st);
     if (int rc = network_energy_forces(m, pos, m->md_species.as<int32_t>(), N, m->md_E.as<double>(), F, nullptr, st)) return rc;
+    prof_begin(m, st, KC_MD, 0);
     k_kick_drift<<<g3, T, 0, st>>>(pos, vel, F, m->md_mass.as<double>(), N, dt, 0);
+    prof_end(m, st);
     m->launches += 2;
   }
   m->stats[4] += n_steps;

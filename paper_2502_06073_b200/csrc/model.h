@@ -62,8 +62,21 @@ struct Workspace {       // per-chunk activations, sized for cap_edges active ed
   float* yb = nullptr; float* ub = nullptr; float* bb = nullptr; float* gammab = nullptr;
 };
 
+// optional per-kernel-class timing with CUDA events on the launching stream (allegro_profile)
+enum { KC_GEMM = 0, KC_TP_FWD, KC_TP_BWD, KC_GAMMA, KC_GAMMABAR, KC_ACTIVE, KC_EDGE_MISC, KC_NEIGHBOR, KC_MD, KC_GATHER, KC_COUNT };
+struct Prof {
+  bool on = false;
+  std::vector<cudaEvent_t> ev;      // pairs
+  std::vector<int> cls;             // class of each pair
+  size_t used = 0;                  // pairs in flight
+  double ms[KC_COUNT] = {0};
+  int64_t launches[KC_COUNT] = {0};
+  double work[KC_COUNT] = {0};      // class-specific work units: GEMM/TP = flops per active edge, summed over launches
+};
+
 struct Model {
   Plan plan;
+  Prof prof;
   std::string err;
   int device = 0;
   int num_sms = 148;
@@ -84,6 +97,10 @@ struct Model {
 // device flag slots (int32 array in Model::flags)
 enum { FLAG_REBUILD = 0, FLAG_ERR_SHIFT = 1, FLAG_ERR_CAP = 2, FLAG_STALE = 3, FLAG_NONFINITE = 4, FLAG_SPECIES = 5,
        FLAG_NREBUILD = 6, FLAG_COUNT = 16 };
+
+// ---- profiling brackets (api.cu)
+void prof_begin(Model* m, cudaStream_t st, int cls, double work);
+void prof_end(Model* m, cudaStream_t st);
 
 // ---- helpers (api.cu)
 int ensure(Model* m, DevBuf* b, size_t bytes);            // grow-only cudaMalloc; 0 or ALLEGRO_ERR_ALLOC

@@ -98,6 +98,19 @@ int ws_prepare(Model* m, int64_t cap_edges, int64_t cap_atoms) {
   return 0;
 }
 
+// algorithmic flop per active edge of one layer's tensor product (+ channel mixing): 3 flop per coupling nonzero
+// and channel, 2 n^2 (2l+1) per path through W_lin; the backward has two coupling products.
+static double tp_work(const Plan& P, int L, bool backward) {
+  const Layer& ly = P.layers[L - 1];
+  const double n = P.hp.n_channels;
+  double f = 0;
+  for (const Path& p : ly.paths) {
+    f += (backward ? 6.0 : 3.0) * n * (p.cg_end - p.cg_begin);
+    if (L < P.hp.n_layers) f += 2.0 * n * n * (2 * ly.out_irreps[p.iro].l + 1);
+  }
+  return f;
+}
+
 static TpLayerDev make_tp(const Model* m, int L) {
   const Plan& P = m->plan;
   const Layer& ly = P.layers[L - 1];
@@ -126,11 +139,13 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
   const int T = 256;
   const unsigned gridWA = (unsigned)((na * 32 + T - 1) / T);
   // ---- active edges of the chunk
+  prof_begin(m, st, KC_ACTIVE, 0);
   k_active<0><<<gridWA, T, 0, st>>>(pos, species, lv, a0, a1, hp.r_cut, hp.poly_p, Nb, ws.act_cnt, nullptr, nullptr, nullptr, nullptr,
                                     nullptr, nullptr, nullptr, 0, flags);
   if (int rc = scan_counts(m, ws.act_cnt, ws.rowptr_c, na, &ws.scan_tmp, nullptr, st)) return rc;
   k_active<1><<<gridWA, T, 0, st>>>(pos, species, lv, a0, a1, hp.r_cut, hp.poly_p, Nb, nullptr, ws.rowptr_c, ws.e_center, ws.e_j,
                                     ws.e_lidx, ws.geo, ws.bes, m->g_list.as<float>(), ws.cap_edges, flags);
+  prof_end(m, st);
   m->launches += 2;
   const int64_t* Mptr = ws.rowptr_c + na;
   const float* w = m->d_w;
@@ -175,7 +190,9 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
       launch_gemm(m, g, m_cap, st);
     }
     // F7
+    prof_begin(m, st, KC_GAMMA, 0);
     k_gamma<<<(unsigned)na, 128, 0, st>>>(ws.rowptr_c, ws.geo, ws.wenv[L - 1], ldw_env, n, hp.lmax, inv_sqrt_navg, ws.gamma[L - 1], na);
+    prof_end(m, st);
     // F8, F9, F11
     int d3max = 1;
     for (int o = 0; o < tp.n_out; ++o) if (tp.has_lin || o == 0) d3max = std::max(d3max, tp.out_d3[o]);
@@ -191,7 +208,9 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
       size_t smem = (size_t)(n * TE * d3max + n * n + TE * 16) * sizeof(float);
       cudaFuncSetAttribute(k_tp_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
       dim3 grid((unsigned)((m_cap + TE - 1) / TE), (unsigned)(tp.has_lin ? tp.n_out : 1));
+      prof_begin(m, st, KC_TP_FWD, tp_work(P, L, false));
       k_tp_fwd<<<grid, TP_T, smem, st>>>(tp, io, TE);
+      prof_end(m, st);
     }
     m->launches += 2;
     // F10: latent MLP on (x | s), residual update
@@ -210,13 +229,17 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
     }
   }
   // ---- F12
+  prof_begin(m, st, KC_EDGE_MISC, 0);
   k_readout<<<gridWA, T, 0, st>>>(ws.rowptr_c, ws.x[NL], D, m->d_weff, species, a0, na, w + P.w_sigma, w + P.w_mu, m->e_atom.as<float>());
+  prof_end(m, st);
   m->launches += 1;
 
   // ================= backward =================
   cudaMemsetAsync(ws.yb, 0, sizeof(float) * (size_t)m_cap * dsh, st);
+  prof_begin(m, st, KC_EDGE_MISC, 0);
   k_xbar_init<<<(unsigned)((m_cap * D + T - 1) / T), T, 0, st>>>(Mptr, ws.geo, w + P.w_sigma, m->d_weff, D, ws.xb[0]);   // B1
   m->launches += 1;
+  prof_end(m, st);
   int xcur = 0, vcur = 0;
   bool ub_init = false;
   for (int L = NL; L >= 1; --L) {
@@ -224,7 +247,9 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
     const TpLayerDev& tp = tps[L - 1];
     const float c_old = m->c_old[L - 1], c_new = m->c_new[L - 1];
     // B3: ubar += c_new (xbar . y)
+    prof_begin(m, st, KC_EDGE_MISC, 0);
     k_rowdot<<<gridWE, T, 0, st>>>(Mptr, ws.xb[xcur], ws.ylat[L - 1], D, c_new, ub_init ? 1 : 0, ws.ub);
+    prof_end(m, st);
     ub_init = true;
     m->launches += 1;
     // B3/B4: latent MLP backward.  ybar = c_new u xbar is applied as the prologue of the first transposed GEMM.
@@ -261,7 +286,9 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
       io.sbar = ws.sb; io.vbar = (L < NL) ? ws.vb[vcur] : nullptr; io.vbar_prev = ws.vb[vcur ^ 1]; io.ge = ws.ge;
       size_t smem = smem_of(TE);
       cudaFuncSetAttribute(k_tp_bwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      prof_begin(m, st, KC_TP_BWD, tp_work(P, L, true));
       k_tp_bwd<<<(unsigned)((m_cap + TE - 1) / TE), TP_T, smem, st>>>(tp, io, TE, d3max);
+      prof_end(m, st);
       vcur ^= 1;
       m->launches += 1;
     }
@@ -269,8 +296,10 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
     const int ldw_env = (L == 1) ? 2 * nsc : nsc;
     float* wbar = (L == 1) ? ws.wb + nsc : ws.wb;
     const int ldwb = (L == 1) ? 2 * nsc : nsc;
+    prof_begin(m, st, KC_GAMMABAR, 0);
     k_gammabar<<<(unsigned)na, 128, (size_t)(n * dsh + 16) * sizeof(float), st>>>(ws.rowptr_c, ws.geo, ws.ge, ws.wenv[L - 1], ldw_env, n,
                                                                                   hp.lmax, inv_sqrt_navg, wbar, ldwb, ws.yb, na);
+    prof_end(m, st);
     m->launches += 1;
     if (L >= 2) {   // B7: xbar^{L-1} += W_env^T wbar
       g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo; g.wtrans = 1;
@@ -279,12 +308,16 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
     }
   }
   // B8: adjoint of V^0, then [W_init; W_env^1]^T [wbar_init; wbar^1] in one GEMM (B7 of layer 1 + B8)
+  prof_begin(m, st, KC_EDGE_MISC, 0);
   k_init_bwd<<<gridWE, T, 0, st>>>(Mptr, ws.geo, ws.vb[vcur], ws.winit_w1, 2 * nsc, n, hp.lmax, ws.wb, 2 * nsc, ws.yb);
+  prof_end(m, st);
   g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo; g.wtrans = 1;
   g.A0 = ws.wb; g.lda0 = g.K0 = 2 * nsc; g.W = w + P.w_init; g.ldw = D; g.N = D; g.C = ws.xb[xcur]; g.ldc = D; g.epi = EPI_ACCUM;
   launch_gemm(m, g, m_cap, st);
   // B9: ubar += xbar0 . y0;  two-body MLP backward with ybar0 = u xbar0
+  prof_begin(m, st, KC_EDGE_MISC, 0);
   k_rowdot<<<gridWE, T, 0, st>>>(Mptr, ws.xb[xcur], ws.y0, D, 1.0f, 1, ws.ub);
+  prof_end(m, st);
   m->launches += 2;
   {
     const float* cur = ws.xb[xcur];
@@ -305,7 +338,9 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
     launch_gemm(m, g, m_cap, st);
   }
   // B10, B11
+  prof_begin(m, st, KC_EDGE_MISC, 0);
   k_edge_grad<<<gridE, T, 0, st>>>(Mptr, ws.geo, ws.bes, ws.bb, ws.ub, ws.yb, ws.e_lidx, Nb, hp.lmax, (float)hp.r_cut, m->g_list.as<float>());
+  prof_end(m, st);
   m->launches += 1;
   return 0;
 }
@@ -340,10 +375,12 @@ int network_energy_forces(Model* m, const double* pos, const int32_t* species, i
   }
   ListView lv{nl.rowptr.as<int64_t>(), nl.keys.as<uint64_t>(), nl.revpos.as<int>(), {nl.L[0], nl.L[1], nl.L[2]}};
   if (N > 0) {
+    prof_begin(m, st, KC_GATHER, 0);
     k_force_gather<<<(unsigned)((N * 32 + T - 1) / T), T, 0, st>>>(lv, N, m->g_list.as<float>(), F_out, flags);
     const int nb = (int)std::min<int64_t>(1024, (N + 255) / 256);
     k_energy_partial<<<nb, 256, 0, st>>>(m->e_atom.as<float>(), N, m->e_partial.as<double>());
     k_energy_final<<<1, 256, 0, st>>>(m->e_partial.as<double>(), nb, E_out, flags);
+    prof_end(m, st);
     m->launches += 3;
   } else {
     cudaMemsetAsync(E_out, 0, sizeof(double), st);
