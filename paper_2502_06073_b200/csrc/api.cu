@@ -1,5 +1,6 @@
 // api.cu — the C-ABI entry points declared in include/allegro.h (argument checking, ownership, error codes).
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -139,6 +140,7 @@ int allegro_create(const float* weights_host, size_t n_weights, const allegro_hp
     delete m; return ALLEGRO_ERR_CUDA;
   }
   cudaGetDevice(&m->device);
+  { const char* g = std::getenv("ALLEGRO_GEMM"); m->use_tc = !(g && std::string(g) == "fp32"); }
   cudaDeviceGetAttribute(&m->num_sms, cudaDevAttrMultiProcessorCount, m->device);
   auto fail = [&](int rc, const std::string& msg) { g_create_err = msg; allegro_destroy(m); return rc; };
   if (cudaMalloc(&m->d_w, sizeof(float) * std::max<size_t>(n_weights, 1)) != cudaSuccess) return fail(ALLEGRO_ERR_ALLOC, "weights allocation failed");

@@ -31,9 +31,31 @@ struct GemmArgs {
   int split = 0;                     // EPI_SPLIT_RES: columns < split -> C (residual), >= split -> C2
 };
 
+// one output element through the fused epilogue
+__device__ __forceinline__ void gemm_epi(const GemmArgs& a, int64_t row, int n, float v, float u, int zi, int zj) {
+  switch (a.epi) {
+    case EPI_STORE: a.C[row * a.ldc + n] = v; break;
+    case EPI_GATHER2:
+      a.C[row * a.ldc + n] = v + a.Wg[(int64_t)n * a.ldwg + zi] + a.Wg[(int64_t)n * a.ldwg + a.S + zj];
+      break;
+    case EPI_Y_X:
+      a.C[row * a.ldc + n] = v; a.C2[row * a.ldc2 + n] = u * v; break;
+    case EPI_RESIDUAL:
+      a.C[row * a.ldc + n] = v;
+      a.C2[row * a.ldc2 + n] = a.c_old * a.aux[row * a.ldaux + n] + a.c_new * u * v;
+      break;
+    case EPI_DSILU: a.C[row * a.ldc + n] = v * dsilu_f(a.aux[row * a.ldaux + n]); break;
+    case EPI_ACCUM: a.C[row * a.ldc + n] += v; break;
+    case EPI_SPLIT_RES:
+      if (n < a.split) a.C[row * a.ldc + n] = a.c_old * a.aux[row * a.ldaux + n] + v;
+      else a.C2[row * a.ldc2 + (n - a.split)] = v;
+      break;
+  }
+}
+
 constexpr int GM = 128, GN = 64, GK = 16, GT = 256;
 
-__global__ void __launch_bounds__(GT) k_gemm(GemmArgs a) {
+static __global__ void __launch_bounds__(GT) k_gemm(GemmArgs a) {
   __shared__ __align__(16) float As[GK][GM + 4];
   __shared__ __align__(16) float Bs[GK][GN + 4];
   const int64_t M = *a.Mptr;
@@ -129,31 +151,16 @@ __global__ void __launch_bounds__(GT) k_gemm(GemmArgs a) {
     for (int j = 0; j < 4; ++j) {
       const int n = col0 + tx * 4 + j;
       if (n >= a.N) continue;
-      float v = acc[i][j];
-      switch (a.epi) {
-        case EPI_STORE: a.C[row * a.ldc + n] = v; break;
-        case EPI_GATHER2:
-          a.C[row * a.ldc + n] = v + a.Wg[(int64_t)n * a.ldwg + zi] + a.Wg[(int64_t)n * a.ldwg + a.S + zj];
-          break;
-        case EPI_Y_X:
-          a.C[row * a.ldc + n] = v; a.C2[row * a.ldc2 + n] = u * v; break;
-        case EPI_RESIDUAL:
-          a.C[row * a.ldc + n] = v;
-          a.C2[row * a.ldc2 + n] = a.c_old * a.aux[row * a.ldaux + n] + a.c_new * u * v;
-          break;
-        case EPI_DSILU: a.C[row * a.ldc + n] = v * dsilu_f(a.aux[row * a.ldaux + n]); break;
-        case EPI_ACCUM: a.C[row * a.ldc + n] += v; break;
-        case EPI_SPLIT_RES:
-          if (n < a.split) a.C[row * a.ldc + n] = a.c_old * a.aux[row * a.ldaux + n] + v;
-          else a.C2[row * a.ldc2 + (n - a.split)] = v;
-          break;
-      }
+      gemm_epi(a, row, n, acc[i][j], u, zi, zj);
     }
   }
 }
 
+void launch_gemm_tc(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st);   // gemm_tc.cu
+
 inline void launch_gemm(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st) {
   if (m_cap <= 0) return;
+  if (m->use_tc) { launch_gemm_tc(m, a, m_cap, st); return; }
   dim3 grid((unsigned)((m_cap + GM - 1) / GM), (unsigned)((a.N + GN - 1) / GN));
   prof_begin(m, st, KC_GEMM, 2.0 * a.N * (a.K0 + a.K1));
   k_gemm<<<grid, GT, 0, st>>>(a);

@@ -80,6 +80,7 @@ struct Model {
   std::string err;
   int device = 0;
   int num_sms = 148;
+  bool use_tc = true;              // dense linears on tcgen05 (3xTF32); ALLEGRO_GEMM=fp32 selects the FP32-pipe kernel
   float* d_w = nullptr;            // weight blob
   float* d_weff = nullptr;         // collapsed edge-energy chain W_last...W_1 -> [D]
   std::vector<CgDev> cg;           // per layer
