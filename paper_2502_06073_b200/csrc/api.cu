@@ -203,6 +203,7 @@ int allegro_destroy(void* h) {
   if (m->d_w) cudaFree(m->d_w);
   if (m->d_weff) cudaFree(m->d_weff);
   for (cudaEvent_t e : m->prof.ev) cudaEventDestroy(e);
+  for (auto& kv : m->packed_w) if (kv.second) cudaFree(kv.second);
   for (CgDev& c : m->cg) { if (c.path_tab) cudaFree(c.path_tab); if (c.cg_idx) cudaFree(c.cg_idx); if (c.cg_val) cudaFree(c.cg_val); }
   NeighborList& nl = m->nl;
   for (DevBuf* b : {&nl.r_build, &nl.img, &nl.cell_of, &nl.cell_cnt, &nl.cell_start, &nl.cell_fill, &nl.sorted, &nl.row_cnt, &nl.rowptr,

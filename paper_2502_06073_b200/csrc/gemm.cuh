@@ -53,6 +53,50 @@ __device__ __forceinline__ void gemm_epi(const GemmArgs& a, int64_t row, int n, 
   }
 }
 
+// four consecutive output columns n..n+3 (n % 4 == 0, all < N, every leading dimension a multiple of 4)
+__device__ __forceinline__ void gemm_epi4(const GemmArgs& a, int64_t row, int n, float4 v, float u, int zi, int zj) {
+  auto ld4 = [](const float* p) { return *reinterpret_cast<const float4*>(p); };
+  auto st4 = [](float* p, float4 x) { *reinterpret_cast<float4*>(p) = x; };
+  switch (a.epi) {
+    case EPI_STORE: st4(a.C + row * a.ldc + n, v); break;
+    case EPI_GATHER2: {
+      const float* g = a.Wg + (int64_t)n * a.ldwg;
+      v.x += g[zi] + g[a.S + zj]; g += a.ldwg;
+      v.y += g[zi] + g[a.S + zj]; g += a.ldwg;
+      v.z += g[zi] + g[a.S + zj]; g += a.ldwg;
+      v.w += g[zi] + g[a.S + zj];
+      st4(a.C + row * a.ldc + n, v);
+    } break;
+    case EPI_Y_X:
+      st4(a.C + row * a.ldc + n, v);
+      st4(a.C2 + row * a.ldc2 + n, make_float4(u * v.x, u * v.y, u * v.z, u * v.w));
+      break;
+    case EPI_RESIDUAL: {
+      st4(a.C + row * a.ldc + n, v);
+      const float4 x = ld4(a.aux + row * a.ldaux + n);
+      const float cu = a.c_new * u;
+      st4(a.C2 + row * a.ldc2 + n, make_float4(a.c_old * x.x + cu * v.x, a.c_old * x.y + cu * v.y, a.c_old * x.z + cu * v.z,
+                                               a.c_old * x.w + cu * v.w));
+    } break;
+    case EPI_DSILU: {
+      const float4 z = ld4(a.aux + row * a.ldaux + n);
+      st4(a.C + row * a.ldc + n, make_float4(v.x * dsilu_f(z.x), v.y * dsilu_f(z.y), v.z * dsilu_f(z.z), v.w * dsilu_f(z.w)));
+    } break;
+    case EPI_ACCUM: {
+      const float4 c = ld4(a.C + row * a.ldc + n);
+      st4(a.C + row * a.ldc + n, make_float4(c.x + v.x, c.y + v.y, c.z + v.z, c.w + v.w));
+    } break;
+    case EPI_SPLIT_RES:
+      if (n < a.split) {
+        const float4 x = ld4(a.aux + row * a.ldaux + n);
+        st4(a.C + row * a.ldc + n, make_float4(a.c_old * x.x + v.x, a.c_old * x.y + v.y, a.c_old * x.z + v.z, a.c_old * x.w + v.w));
+      } else {
+        st4(a.C2 + row * a.ldc2 + (n - a.split), v);
+      }
+      break;
+  }
+}
+
 constexpr int GM = 128, GN = 64, GK = 16, GT = 256;
 
 static __global__ void __launch_bounds__(GT) k_gemm(GemmArgs a) {

@@ -9,15 +9,18 @@
 //   a = a_hi + a_lo (a_hi = rna-rounded TF32),  A B ~= A_hi B_hi + A_hi B_lo + A_lo B_hi   (fp32 accumulation in TMEM)
 // leaves ~2^-21 relative error per product, the same class as fp32 FMA.
 //
-// Structure of one CTA (128 threads, one 128-row tile of edges x up to 128 output columns):
-//   * the four warps stage a 128 x 32 slice of A (prologue applied, split into hi/lo) and the matching N x 32 slice of B
-//     (weights, split into hi/lo) in shared memory in the canonical K-major no-swizzle UMMA layout
-//     [row/8][k/4][row%8][k%4] (core matrix = 8 rows x 16 B; LBO = 128 B between the k-chunks, SBO = 1024 B between
-//     8-row groups), two stages;
-//   * one elected thread issues 3 x 4 tcgen05.mma.cta_group::1.kind::tf32 (M=128, N, K=8) per slice and commits them to
+// Structure of one CTA (256 threads, one 128-row tile of edges x up to 128 output columns; three CTAs fit on an SM):
+//   * B (the weight block) is split into hi/lo and laid out in the canonical K-major no-swizzle UMMA layout ONCE per
+//     call site (k_pack_w, cached in the handle); per 16-deep k slice one thread pulls its 2 x N x 16 block into shared
+//     memory with a single cp.async.bulk that completes on the stage's mbarrier;
+//   * the eight warps stage the 128 x 16 slice of A (prologue applied, hi/lo split) in the same canonical layout
+//     [row/8][k/4][row%8][k%4] (core matrix = 8 rows x 16 B; LBO = 128 B between k-chunks, SBO = 512 B between 8-row
+//     groups), two stages;
+//   * one elected thread issues 3 x 2 tcgen05.mma.cta_group::1.kind::tf32 (M=128, N, K=8) per slice and commits them to
 //     the stage's mbarrier, so the next slice is staged while the tensor pipe runs;
 //   * accumulators live in TMEM (N fp32 columns x 128 lanes); the epilogue reads them with tcgen05.ld.32x32b (one
-//     output row per thread) and applies the fused epilogue while writing to global memory.
+//     output row per thread, two warps per lane quadrant taking alternate 16-column groups) and applies the fused
+//     epilogue with 128-bit stores.
 #include <cstdint>
 
 #include "gemm.cuh"
@@ -25,7 +28,7 @@
 namespace allegro {
 namespace {
 
-constexpr int TC_M = 128, TC_KC = 32, TC_T = 128, TC_NMAX = 128;
+constexpr int TC_M = 128, TC_KC = 16, TC_T = 256, TC_NMAX = 128;
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -83,10 +86,34 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float* v) {
   for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
 }
 
-// smem layout per stage: A_hi | A_lo (128 x 32 fp32 each = 16 KB) | B_hi | B_lo (Npad x 32 fp32 each)
-__global__ void __launch_bounds__(TC_T) k_gemm_tc(GemmArgs a, int Npad, int tmem_cols) {
+__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
+               "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+
+// Packed B operand: for each 128-column tile, for each k slice: [hi block | lo block], block = Nt x 16 fp32 canonical.
+__global__ void k_pack_w(const float* __restrict__ W, int ldw, int wtrans, int N, int K, int Npad, int Kpad, float* __restrict__ out) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (int64_t)Npad * Kpad) return;
+  const int n = (int)(idx / Kpad), k = (int)(idx - (int64_t)n * Kpad);
+  float v = 0.f;
+  if (n < N && k < K) v = wtrans ? W[(int64_t)k * ldw + n] : W[(int64_t)n * ldw + k];
+  const float hi = tf32_rna(v), lo = v - hi;
+  const int tile = n / TC_NMAX, nl = n - tile * TC_NMAX, Nt = min(Npad - tile * TC_NMAX, TC_NMAX);
+  const int c = k / TC_KC, kl = k - c * TC_KC;
+  const int64_t base = (int64_t)tile * TC_NMAX * Kpad * 2 + (int64_t)c * (2 * Nt * TC_KC);
+  const int off = (nl >> 3) * (TC_KC / 4) * 32 + (kl >> 2) * 32 + (nl & 7) * 4 + (kl & 3);
+  out[base + off] = hi;
+  out[base + Nt * TC_KC + off] = lo;
+}
+
+// smem per stage: A_hi | A_lo (128 x 16 fp32 each = 8 KB) | B_hi | B_lo (Nt x 16 fp32 each)
+__global__ void __launch_bounds__(TC_T) k_gemm_tc(GemmArgs a, const float* __restrict__ Bp, int Npad, int Kpad, int tmem_cols, int vec_ok) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
-  __shared__ __align__(8) uint64_t mbar[2];
+  __shared__ __align__(8) uint64_t mbar_mma[2];
+  __shared__ __align__(8) uint64_t mbar_b[2];
   __shared__ uint32_t tmem_base_s;
   const int64_t M = *a.Mptr;
   const int64_t row0 = (int64_t)blockIdx.x * TC_M;
@@ -95,138 +122,126 @@ __global__ void __launch_bounds__(TC_T) k_gemm_tc(GemmArgs a, int Npad, int tmem
   const int Nt = min(Npad - col0, TC_NMAX);           // columns of this tile (multiple of 16)
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int K = a.K0 + a.K1;
-  const int nchunks = (K + TC_KC - 1) / TC_KC;
-  const uint32_t a_bytes = TC_M * TC_KC * 4, b_bytes = (uint32_t)Nt * TC_KC * 4;
+  const int nchunks = Kpad / TC_KC;
+  constexpr uint32_t a_bytes = TC_M * TC_KC * 4;
+  const uint32_t b_bytes = (uint32_t)Nt * TC_KC * 4;
   const uint32_t stage_bytes = 2 * a_bytes + 2 * b_bytes;
-  uint8_t* sm = smem_raw;
+  const float* Bt = Bp + (int64_t)blockIdx.y * TC_NMAX * Kpad * 2;
 
   if (warp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "r"(tmem_cols));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
   if (tid == 0) {
-    mbar_init(&mbar[0], 1); mbar_init(&mbar[1], 1);
+    mbar_init(&mbar_mma[0], 1); mbar_init(&mbar_mma[1], 1);
+    mbar_init(&mbar_b[0], 1); mbar_init(&mbar_b[1], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
   asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
   const uint32_t tmem_d = tmem_base_s;
-  // instruction descriptor: D fp32, A/B tf32, K-major both, N, M=128
+  // instruction descriptor: D fp32 (bit 4), A/B tf32 (2 at bits 7 and 10), both K-major, N>>3 at bit 17, M>>4 at bit 24
   const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(Nt >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24);
 
-  const int64_t arow = row0 + tid;                    // this thread stages row `tid` of A and column `tid` of B
+  const int r = tid & 127, qh = tid >> 7;              // this thread stages row r, k-quads 2*qh and 2*qh+1 of each slice
+  const int64_t arow = row0 + r;
   const bool arow_ok = arow < M;
   float ascale = 1.f;
   if (a.pro == PRO_SCALE_U && arow_ok) ascale = a.c_new * a.geo[arow * GEO_W + 4];
-  const int bn = col0 + tid;
-  const bool bcol_ok = tid < Nt && bn < a.N;
+  const int off_row = (r >> 3) * (TC_KC / 4) * 32 + (r & 7) * 4;   // floats: (row/8)*SBO + (row%8)*16 B
 
   for (int c = 0; c < nchunks; ++c) {
     const int b = c & 1;
-    if (c >= 2) mbar_wait(&mbar[b], (uint32_t)(((c >> 1) - 1) & 1));   // MMAs of slice c-2 have drained stage b
-    uint8_t* st = sm + (size_t)b * stage_bytes;
+    if (c >= 2) mbar_wait(&mbar_mma[b], (uint32_t)(((c >> 1) - 1) & 1));   // MMAs of slice c-2 have drained stage b
+    uint8_t* st = smem_raw + (size_t)b * stage_bytes;
     float* Ahi = reinterpret_cast<float*>(st);
     float* Alo = reinterpret_cast<float*>(st + a_bytes);
     float* Bhi = reinterpret_cast<float*>(st + 2 * a_bytes);
-    float* Blo = reinterpret_cast<float*>(st + 2 * a_bytes + b_bytes);
+    if (tid == 0) bulk_g2s(Bhi, Bt + (int64_t)c * (2 * Nt * TC_KC), 2 * b_bytes, &mbar_b[b]);
     const int k0 = c * TC_KC;
-    // ---- A slice: row `tid`, 8 quads of k
-    {
-      const int off_row = (tid >> 3) * (TC_KC / 4) * 32 + (tid & 7) * 4;   // floats: (row/8)*SBO + (row%8)*16B
 #pragma unroll
-      for (int q = 0; q < TC_KC / 4; ++q) {
-        const int kk = k0 + q * 4;
-        float v[4] = {0.f, 0.f, 0.f, 0.f};
-        if (arow_ok && kk < K) {
-          const float* src; int kl, kmax;
-          if (kk < a.K0) { src = a.A0 + arow * a.lda0; kl = kk; kmax = a.K0; }
-          else { src = a.A1 + arow * a.lda1; kl = kk - a.K0; kmax = a.K1; }
-          if (kl + 3 < kmax && ((((uintptr_t)(src + kl)) & 15) == 0)) {
-            const float4 t = *reinterpret_cast<const float4*>(src + kl);
-            v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
-          } else {
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-              const int kq = kk + e;
-              if (kq < K) v[e] = (kq < a.K0) ? a.A0[arow * a.lda0 + kq] : a.A1[arow * a.lda1 + (kq - a.K0)];
-            }
-          }
-          if (a.pro == PRO_SILU) {
-#pragma unroll
-            for (int e = 0; e < 4; ++e) v[e] = silu_f(v[e]);
-          } else if (a.pro == PRO_SCALE_U) {
-#pragma unroll
-            for (int e = 0; e < 4; ++e) v[e] *= ascale;
-          }
-        }
-        float4 hi, lo;
-        hi.x = tf32_rna(v[0]); hi.y = tf32_rna(v[1]); hi.z = tf32_rna(v[2]); hi.w = tf32_rna(v[3]);
-        lo.x = v[0] - hi.x; lo.y = v[1] - hi.y; lo.z = v[2] - hi.z; lo.w = v[3] - hi.w;
-        *reinterpret_cast<float4*>(Ahi + off_row + q * 32) = hi;
-        *reinterpret_cast<float4*>(Alo + off_row + q * 32) = lo;
-      }
-    }
-    // ---- B slice: output column `tid` (B is K-major: rows = n, contiguous along k)
-    if (tid < Nt) {
-      const int off_row = (tid >> 3) * (TC_KC / 4) * 32 + (tid & 7) * 4;
-#pragma unroll
-      for (int q = 0; q < TC_KC / 4; ++q) {
-        float v[4] = {0.f, 0.f, 0.f, 0.f};
-        if (bcol_ok) {
+    for (int qq = 0; qq < 2; ++qq) {
+      const int q = qh * 2 + qq;
+      const int kk = k0 + q * 4;
+      float v[4] = {0.f, 0.f, 0.f, 0.f};
+      if (arow_ok && kk < K) {
+        const float* src; int kl, kmax;
+        if (kk < a.K0) { src = a.A0 + arow * a.lda0; kl = kk; kmax = a.K0; }
+        else { src = a.A1 + arow * a.lda1; kl = kk - a.K0; kmax = a.K1; }
+        if (kl + 3 < kmax && ((((uintptr_t)(src + kl)) & 15) == 0)) {
+          const float4 t = *reinterpret_cast<const float4*>(src + kl);
+          v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+        } else {
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
-            const int kk = k0 + q * 4 + e;
-            if (kk < K) v[e] = a.wtrans ? a.W[(int64_t)kk * a.ldw + bn] : a.W[(int64_t)bn * a.ldw + kk];
+            const int kq = kk + e;
+            if (kq < K) v[e] = (kq < a.K0) ? a.A0[arow * a.lda0 + kq] : a.A1[arow * a.lda1 + (kq - a.K0)];
           }
         }
-        float4 hi, lo;
-        hi.x = tf32_rna(v[0]); hi.y = tf32_rna(v[1]); hi.z = tf32_rna(v[2]); hi.w = tf32_rna(v[3]);
-        lo.x = v[0] - hi.x; lo.y = v[1] - hi.y; lo.z = v[2] - hi.z; lo.w = v[3] - hi.w;
-        *reinterpret_cast<float4*>(Bhi + off_row + q * 32) = hi;
-        *reinterpret_cast<float4*>(Blo + off_row + q * 32) = lo;
+        if (a.pro == PRO_SILU) {
+#pragma unroll
+          for (int e = 0; e < 4; ++e) v[e] = silu_f(v[e]);
+        } else if (a.pro == PRO_SCALE_U) {
+#pragma unroll
+          for (int e = 0; e < 4; ++e) v[e] *= ascale;
+        }
       }
+      float4 hi, lo;
+      hi.x = tf32_rna(v[0]); hi.y = tf32_rna(v[1]); hi.z = tf32_rna(v[2]); hi.w = tf32_rna(v[3]);
+      lo.x = v[0] - hi.x; lo.y = v[1] - hi.y; lo.z = v[2] - hi.z; lo.w = v[3] - hi.w;
+      *reinterpret_cast<float4*>(Ahi + off_row + q * 32) = hi;
+      *reinterpret_cast<float4*>(Alo + off_row + q * 32) = lo;
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy smem writes -> visible to the tensor core
     __syncthreads();
     if (tid == 0) {
+      mbar_wait(&mbar_b[b], (uint32_t)((c >> 1) & 1));             // the weight block of this slice has landed
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-      const uint32_t sa_hi = smem_u32(Ahi), sa_lo = smem_u32(Alo), sb_hi = smem_u32(Bhi), sb_lo = smem_u32(Blo);
-      const int ksteps = min(TC_KC, (K - k0 + 7) / 8 * 8) / 8;   // K=8 steps that hold real data
-      const uint32_t sbo = (TC_KC / 4) * 128;   // bytes between 8-row groups
-      for (int ks = 0; ks < ksteps; ++ks) {
-        const uint32_t koff = ks * 256;          // two 128-byte k-chunks per K=8 step
+      const uint32_t sa_hi = smem_u32(Ahi), sa_lo = smem_u32(Alo), sb_hi = smem_u32(Bhi), sb_lo = sb_hi + b_bytes;
+      constexpr uint32_t sbo = (TC_KC / 4) * 128;                   // bytes between 8-row groups
+#pragma unroll
+      for (int ks = 0; ks < TC_KC / 8; ++ks) {
+        const uint32_t koff = ks * 256;                              // two 128-byte k-chunks per K=8 step
         const uint64_t dAh = umma_desc(sa_hi + koff, 128, sbo), dAl = umma_desc(sa_lo + koff, 128, sbo);
         const uint64_t dBh = umma_desc(sb_hi + koff, 128, sbo), dBl = umma_desc(sb_lo + koff, 128, sbo);
         umma_tf32(tmem_d, dAl, dBh, idesc, (c > 0 || ks > 0) ? 1u : 0u);   // small terms first
         umma_tf32(tmem_d, dAh, dBl, idesc, 1u);
         umma_tf32(tmem_d, dAh, dBh, idesc, 1u);
       }
-      umma_commit(&mbar[b]);
+      umma_commit(&mbar_mma[b]);
     }
   }
-  // all slices issued: wait for the last commit (commits complete in order)
-  {
+  {   // all slices issued: wait for the last commit (commits complete in order)
     const int c = nchunks - 1;
-    mbar_wait(&mbar[c & 1], (uint32_t)((c >> 1) & 1));
+    mbar_wait(&mbar_mma[c & 1], (uint32_t)((c >> 1) & 1));
   }
   asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 
-  // ---- epilogue: thread -> output row (TMEM lane 32*warp + lane)
-  const int64_t row = row0 + tid;
+  // ---- epilogue: thread -> output row (TMEM lane quadrant = warp % 4), warps w and w+4 alternate 16-column groups
+  const int quad = warp & 3, half = warp >> 2;
+  const int64_t row = row0 + quad * 32 + lane;
   float u = 0.f; int zi = 0, zj = 0;
   if (row < M) {
     if (a.epi == EPI_Y_X || a.epi == EPI_RESIDUAL) u = a.geo[row * GEO_W + 4];
     if (a.epi == EPI_GATHER2) { zi = __float_as_int(a.geo[row * GEO_W + 6]); zj = __float_as_int(a.geo[row * GEO_W + 7]); }
   }
-  for (int n0 = 0; n0 < Nt; n0 += 16) {
+  for (int n0 = half * 16; n0 < Nt; n0 += 32) {
     float v[16];
-    tmem_ld16(tmem_d + ((uint32_t)(warp * 32) << 16) + (uint32_t)n0, v);
+    tmem_ld16(tmem_d + ((uint32_t)(quad * 32) << 16) + (uint32_t)n0, v);
     if (row < M) {
+      if (vec_ok) {
 #pragma unroll
-      for (int j = 0; j < 16; ++j) {
-        const int n = col0 + n0 + j;
-        if (n < a.N) gemm_epi(a, row, n, v[j], u, zi, zj);
+        for (int j = 0; j < 16; j += 4) {
+          const int n = col0 + n0 + j;
+          if (n < a.N) gemm_epi4(a, row, n, make_float4(v[j], v[j + 1], v[j + 2], v[j + 3]), u, zi, zj);
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+          const int n = col0 + n0 + j;
+          if (n < a.N) gemm_epi(a, row, n, v[j], u, zi, zj);
+        }
       }
     }
   }
@@ -240,8 +255,21 @@ __global__ void __launch_bounds__(TC_T) k_gemm_tc(GemmArgs a, int Npad, int tmem
 }  // namespace
 
 void launch_gemm_tc(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st) {
-  const int Npad = (a.N + 15) / 16 * 16;
+  const int K = a.K0 + a.K1;
+  const int Npad = (a.N + 15) / 16 * 16, Kpad = (K + TC_KC - 1) / TC_KC * TC_KC;
   const int Nt = std::min(Npad, TC_NMAX);
+  // packed B operand, built once per call site
+  const std::array<int64_t, 5> key = {(int64_t)(a.W - m->d_w), a.ldw, a.wtrans, a.N, K};
+  float* Bp = nullptr;
+  auto it = m->packed_w.find(key);
+  if (it == m->packed_w.end()) {
+    if (cudaMalloc(&Bp, sizeof(float) * 2 * (size_t)Npad * Kpad) != cudaSuccess) { cudaGetLastError(); m->err = "packed weight allocation failed"; return; }
+    const int64_t tot = (int64_t)Npad * Kpad;
+    k_pack_w<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(a.W, a.ldw, a.wtrans, a.N, K, Npad, Kpad, Bp);
+    m->packed_w[key] = Bp;
+  } else {
+    Bp = it->second;
+  }
   int tmem_cols = 32;
   while (tmem_cols < Nt) tmem_cols *= 2;
   const size_t smem = 2 * (size_t)(2 * TC_M * TC_KC * 4 + 2 * Nt * TC_KC * 4);
@@ -250,9 +278,14 @@ void launch_gemm_tc(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st)
     cudaFuncSetAttribute(k_gemm_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * (2 * TC_M * TC_KC * 4 + 2 * TC_NMAX * TC_KC * 4));
     attr_set = true;
   }
+  auto al = [](const void* p) { return ((uintptr_t)p & 15) == 0; };
+  int vec_ok = (a.N % 4 == 0) && (a.ldc % 4 == 0) && al(a.C);
+  if (a.C2) vec_ok = vec_ok && (a.ldc2 % 4 == 0) && al(a.C2);
+  if (a.aux) vec_ok = vec_ok && (a.ldaux % 4 == 0) && al(a.aux);
+  if (a.epi == EPI_SPLIT_RES) vec_ok = vec_ok && (a.split % 4 == 0);
   dim3 grid((unsigned)((m_cap + TC_M - 1) / TC_M), (unsigned)((Npad + TC_NMAX - 1) / TC_NMAX));
-  prof_begin(m, st, KC_GEMM, 2.0 * a.N * (a.K0 + a.K1));
-  k_gemm_tc<<<grid, TC_T, smem, st>>>(a, Npad, tmem_cols);
+  prof_begin(m, st, KC_GEMM, 2.0 * a.N * K);
+  k_gemm_tc<<<grid, TC_T, smem, st>>>(a, Bp, Npad, Kpad, tmem_cols, vec_ok);
   prof_end(m, st);
   m->launches += 1;
 }

@@ -2,7 +2,9 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <array>
 #include <cstdint>
+#include <map>
 #include <string>
 #include <vector>
 
@@ -84,6 +86,7 @@ struct Model {
   float* d_w = nullptr;            // weight blob
   float* d_weff = nullptr;         // collapsed edge-energy chain W_last...W_1 -> [D]
   std::vector<CgDev> cg;           // per layer
+  std::map<std::array<int64_t, 5>, float*> packed_w;   // tcgen05 B operands: hi/lo split, canonical UMMA layout (gemm_tc.cu)
   std::vector<float> c_old, c_new; // host copies
   NeighborList nl;
   Workspace ws;
