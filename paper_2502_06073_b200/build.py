@@ -32,10 +32,18 @@ def build(force: bool = False, verbose: bool = False) -> str:
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     objs = []
     procs = []
-    os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
+    bdir = os.path.join(HERE, "build")
+    os.makedirs(bdir, exist_ok=True)
+    # generated coupling code: host generator built from plan.cpp, run once -> build/tp_gen.cuh
+    gen = os.path.join(bdir, "gen_tp")
+    for cmd in (["g++", "-O1", "-std=c++17", os.path.join(CSRC, "gen_tp.cpp"), os.path.join(CSRC, "plan.cpp"), "-o", gen],
+                [gen, os.path.join(bdir, "tp_gen.cuh")]):
+        r = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+        if r.returncode != 0:
+            raise RuntimeError("tensor-product code generation failed:\n" + r.stdout)
     for src in SOURCES:
         obj = os.path.join(HERE, "build", src.rsplit(".", 1)[0] + ".o")
-        cmd = [nvcc, *NVCC_FLAGS, "-x", "cu", "-c", os.path.join(CSRC, src), "-o", obj]
+        cmd = [nvcc, *NVCC_FLAGS, "-I", bdir, "-x", "cu", "-c", os.path.join(CSRC, src), "-o", obj]
         procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
         objs.append(obj)
     for src, p in procs:

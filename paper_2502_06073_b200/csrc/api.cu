@@ -5,6 +5,7 @@
 #include <new>
 
 #include "model.h"
+#include "tp_gen.cuh"
 
 namespace allegro {
 
@@ -144,7 +145,27 @@ int allegro_create(const float* weights_host, size_t n_weights, const allegro_hp
   cudaDeviceGetAttribute(&m->num_sms, cudaDevAttrMultiProcessorCount, m->device);
   auto fail = [&](int rc, const std::string& msg) { g_create_err = msg; allegro_destroy(m); return rc; };
   if (cudaMalloc(&m->d_w, sizeof(float) * std::max<size_t>(n_weights, 1)) != cudaSuccess) return fail(ALLEGRO_ERR_ALLOC, "weights allocation failed");
-  cudaMemcpy(m->d_w, weights_host, sizeof(float) * n_weights, cudaMemcpyHostToDevice);
+  {
+    // device copy of the blob with the rows of W_init / W_env^L reordered from (c, l) to (l, c): the kernels keep
+    // the channel index fastest in every per-edge tensor (tp.cuh)
+    std::vector<float> wd(weights_host, weights_host + n_weights);
+    const int nl1 = hp->lmax + 1, nch = hp->n_channels;
+    auto permute = [&](int64_t off) {
+      for (int c = 0; c < nch; ++c)
+        for (int l = 0; l < nl1; ++l)
+          std::memcpy(&wd[off + (int64_t)(l * nch + c) * P.D], &weights_host[off + (int64_t)(c * nl1 + l) * P.D], sizeof(float) * P.D);
+    };
+    permute(P.w_init);
+    for (const Layer& ly : P.layers) permute(ly.w_env);
+    cudaMemcpy(m->d_w, wd.data(), sizeof(float) * n_weights, cudaMemcpyHostToDevice);
+  }
+  for (const Layer& ly : P.layers) {
+    const std::string sig = layer_signature(ly, hp->lmax);
+    int id = -1;
+    for (int k = 0; k < tpgen::N_SIGS; ++k) if (sig == tpgen::SIG_STR[k]) id = k;
+    if (id < 0) return fail(ALLEGRO_ERR_UNSUPPORTED, "no generated tensor-product code for layer signature " + sig);
+    m->tp_sig.push_back(id);
+  }
   // collapsed edge-energy chain (no non-linearity): w_eff = W_1^T ... W_last^T, in fp64 on the host
   {
     std::vector<double> v(1, 1.0);   // row vector [1 x width]

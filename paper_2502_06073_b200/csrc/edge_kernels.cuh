@@ -102,9 +102,10 @@ __global__ void k_active(const double* __restrict__ pos, const int* __restrict__
   if (MODE == 0 && lane == 0) act_cnt[a - a0] = total;
 }
 
-// F7: Gamma_i[c, lm] = Nbar^-1/2 sum_{e in row(i)} w[e, c, l] Y_lm(rhat_e).  One block per centre atom; the
-// row's Y are staged in shared memory in slices of 32 edges; each thread owns outputs (c, lm) and sums the row
-// serially in CSR order (deterministic, no atomics).
+// F7: Gamma_i[lm, c] = Nbar^-1/2 sum_{e in row(i)} w[e, l, c] Y_lm(rhat_e).  One block per centre atom; the
+// row's Y are staged in shared memory in slices of 32 edges; each thread owns outputs (lm, c), channel fastest
+// (w[e][l*n + c] and Gamma[a][lm][c] are read/written contiguously), and sums the row serially in CSR order
+// (deterministic, no atomics).
 __global__ void k_gamma(const int64_t* __restrict__ rowptr_c, const float* __restrict__ geo, const float* __restrict__ w, int ldw,
                         int n, int lmax, float inv_sqrt_navg, float* __restrict__ gamma, int64_t n_atoms) {
   const int64_t a = blockIdx.x;
@@ -128,10 +129,10 @@ __global__ void k_gamma(const int64_t* __restrict__ rowptr_c, const float* __res
     for (int q = 0; q < MAXO; ++q) {
       const int o = threadIdx.x + q * blockDim.x;
       if (o < nout) {
-        const int c = o / dsh, lm = o - c * dsh;
+        const int lm = o / n, c = o - lm * n;
         const int l = (lm >= 9) ? 3 : (lm >= 4) ? 2 : (lm >= 1) ? 1 : 0;
         float s = 0.f;
-        for (int t = 0; t < cnt; ++t) s = fmaf(w[(k0 + t) * ldw + c * (lmax + 1) + l], Ys[t][lm], s);
+        for (int t = 0; t < cnt; ++t) s = fmaf(w[(k0 + t) * ldw + l * n + c], Ys[t][lm], s);
         acc[q] += s;
       }
     }
@@ -144,47 +145,58 @@ __global__ void k_gamma(const int64_t* __restrict__ rowptr_c, const float* __res
 }
 
 // B5 (row reduction) + B6: Gammabar_i = sum_row GE[e], then for every edge of the row
-//   wbar[e,c,l] = Nbar^-1/2 sum_m Gammabar[c,l,m] Y_lm(e);   Ybar[e,lm] += Nbar^-1/2 sum_c w[e,c,l] Gammabar[c,lm].
-// One block per centre atom, Gammabar kept in shared memory.
+//   wbar[e,l,c] = Nbar^-1/2 sum_m Gammabar[l,m,c] Y_lm(e);   Ybar[e,lm] += Nbar^-1/2 sum_c w[e,l,c] Gammabar[lm,c].
+// One block per centre atom, Gammabar kept in shared memory ([lm][n+1], padded against bank conflicts).
 __global__ void k_gammabar(const int64_t* __restrict__ rowptr_c, const float* __restrict__ geo, const float* __restrict__ ge,
                            const float* __restrict__ w, int ldw, int n, int lmax, float inv_sqrt_navg,
                            float* __restrict__ wbar, int ldwb, float* __restrict__ ybar, int64_t n_atoms) {
   extern __shared__ float sm[];
   const int64_t a = blockIdx.x;
   if (a >= n_atoms) return;
-  const int dsh = (lmax + 1) * (lmax + 1), nout = n * dsh, nsc = n * (lmax + 1);
-  float* Gb = sm;              // [nout]
-  float* Ys = sm + nout;       // [16]
+  const int dsh = (lmax + 1) * (lmax + 1), nout = n * dsh, ldg = n + 1;
+  float* Gb = sm;              // [dsh][n+1]
   const int64_t b = rowptr_c[a], e = rowptr_c[a + 1];
+  const int len = (int)(e - b);
+  if (len == 0) return;
   for (int o = threadIdx.x; o < nout; o += blockDim.x) {
     float s = 0.f;
     for (int64_t k = b; k < e; ++k) s += ge[k * nout + o];
-    Gb[o] = s * inv_sqrt_navg;
+    const int lm = o / n, c = o - lm * n;
+    Gb[lm * ldg + c] = s * inv_sqrt_navg;
   }
-  for (int64_t k = b; k < e; ++k) {
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      const float* gq = geo + k * GEO_W;
-      sph_harm_rt(lmax, gq[0], gq[1], gq[2], Ys);
+  __syncthreads();
+  // wbar: one (edge, channel) pair per thread and iteration
+  for (int idx = threadIdx.x; idx < len * n; idx += blockDim.x) {
+    const int c = idx % n, kk = idx / n;
+    const int64_t k = b + kk;
+    const float* gq = geo + k * GEO_W;
+    float Y[16];
+    sph_harm_rt(lmax, gq[0], gq[1], gq[2], Y);
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+      if (l <= lmax) {
+        float s = 0.f;
+#pragma unroll
+        for (int mm = 0; mm < 2 * l + 1; ++mm) s = fmaf(Gb[(l * l + mm) * ldg + c], Y[l * l + mm], s);
+        wbar[k * ldwb + l * n + c] = s;
+      }
     }
-    __syncthreads();
-    for (int o = threadIdx.x; o < nsc; o += blockDim.x) {
-      const int c = o / (lmax + 1), l = o - c * (lmax + 1);
-      float s = 0.f;
-      for (int mm = 0; mm < 2 * l + 1; ++mm) s = fmaf(Gb[c * dsh + l * l + mm], Ys[l * l + mm], s);
-      wbar[k * ldwb + o] = s;
-    }
-    if (threadIdx.x < dsh) {
-      const int lm = threadIdx.x;
-      const int l = (lm >= 9) ? 3 : (lm >= 4) ? 2 : (lm >= 1) ? 1 : 0;
-      float s = 0.f;
-      for (int c = 0; c < n; ++c) s = fmaf(w[k * ldw + c * (lmax + 1) + l], Gb[c * dsh + lm], s);
-      ybar[k * dsh + lm] += s;
-    }
+  }
+  // Ybar: one (edge, lm) pair per thread and iteration
+  for (int idx = threadIdx.x; idx < len * dsh; idx += blockDim.x) {
+    const int lm = idx % dsh, kk = idx / dsh;
+    const int64_t k = b + kk;
+    const int l = (lm >= 9) ? 3 : (lm >= 4) ? 2 : (lm >= 1) ? 1 : 0;
+    const float* wk = w + k * ldw + l * n;
+    const float* g = Gb + lm * ldg;
+    float s = 0.f;
+    for (int c = 0; c < n; ++c) s = fmaf(wk[c], g[c], s);
+    ybar[k * dsh + lm] += s;
   }
 }
 
-// B8: wbar_init[e,c,l] = sum_m Vbar0[e,c,l,m] Y_lm;  Ybar[e,lm] += sum_c winit[e,c,l] Vbar0[e,c,lm].  One warp per edge.
+// B8: wbar_init[e,l,c] = sum_m Vbar0[e,lm,c] Y_lm;  Ybar[e,lm] += sum_c winit[e,l,c] Vbar0[e,lm,c].  One warp per edge,
+// lanes over channels (contiguous).
 __global__ void k_init_bwd(const int64_t* __restrict__ Mptr, const float* __restrict__ geo, const float* __restrict__ vbar0,
                            const float* __restrict__ winit, int ldwi, int n, int lmax, float* __restrict__ wbar, int ldwb,
                            float* __restrict__ ybar) {
@@ -198,19 +210,19 @@ __global__ void k_init_bwd(const int64_t* __restrict__ Mptr, const float* __rest
 #pragma unroll
   for (int q = 0; q < 16; ++q) yb[q] = 0.f;
   for (int c = lane; c < n; c += 32) {
-    const float* vb = vbar0 + (e * n + c) * dsh;
+    const float* vb = vbar0 + e * dsh * n + c;
 #pragma unroll
     for (int l = 0; l < 4; ++l) {
       if (l <= lmax) {
-        const float wi = winit[e * ldwi + c * (lmax + 1) + l];
+        const float wi = winit[e * ldwi + l * n + c];
         float s = 0.f;
 #pragma unroll
         for (int mm = 0; mm < 2 * l + 1; ++mm) {
-          const float v = vb[l * l + mm];
+          const float v = vb[(l * l + mm) * n];
           s = fmaf(v, Y[l * l + mm], s);
           yb[l * l + mm] = fmaf(wi, v, yb[l * l + mm]);
         }
-        wbar[e * ldwb + c * (lmax + 1) + l] = s;
+        wbar[e * ldwb + l * n + c] = s;
       }
     }
   }

@@ -86,6 +86,7 @@ struct Model {
   float* d_w = nullptr;            // weight blob
   float* d_weff = nullptr;         // collapsed edge-energy chain W_last...W_1 -> [D]
   std::vector<CgDev> cg;           // per layer
+  std::vector<int> tp_sig;         // per layer: index of the generated coupling code (tp_gen.cuh)
   std::map<std::array<int64_t, 5>, float*> packed_w;   // tcgen05 B operands: hi/lo split, canonical UMMA layout (gemm_tc.cu)
   std::vector<float> c_old, c_new; // host copies
   NeighborList nl;

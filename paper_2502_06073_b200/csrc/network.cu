@@ -111,13 +111,41 @@ static double tp_work(const Plan& P, int L, bool backward) {
   return f;
 }
 
+// launch the generated instantiation of the tensor-product kernels for layer signature `sig`
+static void launch_tp_fwd(int sig, dim3 grid, size_t smem, cudaStream_t st, const TpLayerDev& tp, const TpIo& io, int TE) {
+  static bool attr[tpgen::N_SIGS] = {false};
+  switch (sig) {
+#define X(I)                                                                                                        \
+  case I:                                                                                                           \
+    if (!attr[I]) { cudaFuncSetAttribute(k_tp_fwd<I>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); attr[I] = true; } \
+    k_tp_fwd<I><<<grid, TP_T, smem, st>>>(tp, io, TE);                                                              \
+    break;
+    TPGEN_FOR_EACH_SIG(X)
+#undef X
+    default: break;
+  }
+}
+static void launch_tp_bwd(int sig, dim3 grid, size_t smem, cudaStream_t st, const TpLayerDev& tp, const TpIo& io, int TE, int d3max) {
+  static bool attr[tpgen::N_SIGS] = {false};
+  switch (sig) {
+#define X(I)                                                                                                        \
+  case I:                                                                                                           \
+    if (!attr[I]) { cudaFuncSetAttribute(k_tp_bwd<I>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024); attr[I] = true; } \
+    k_tp_bwd<I><<<grid, TP_T, smem, st>>>(tp, io, TE, d3max);                                                       \
+    break;
+    TPGEN_FOR_EACH_SIG(X)
+#undef X
+    default: break;
+  }
+}
+
 static TpLayerDev make_tp(const Model* m, int L) {
   const Plan& P = m->plan;
   const Layer& ly = P.layers[L - 1];
   TpLayerDev t{};
   t.n = P.hp.n_channels; t.lmax = P.hp.lmax; t.dsh = P.d_sh; t.in_dim = ly.in_dim; t.out_dim = ly.out_dim;
   t.n_paths = (int)ly.paths.size(); t.n_out = (int)ly.out_irreps.size(); t.layer1 = (L == 1); t.has_lin = (L < P.hp.n_layers);
-  t.path_tab = m->cg[L - 1].path_tab; t.cg_idx = m->cg[L - 1].cg_idx; t.cg_val = m->cg[L - 1].cg_val;
+  t.path_tab = m->cg[L - 1].path_tab;
   for (int o = 0; o < t.n_out; ++o) {
     t.out_d3[o] = 2 * ly.out_irreps[o].l + 1; t.out_off[o] = ly.out_off[o]; t.out_np[o] = ly.out_npaths[o];
     t.wlin[o] = ly.w_lin[o];
@@ -199,17 +227,16 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
     d3m[L - 1] = d3max;
     int TE = (16 * TP_T * TP_MAXMT) / (n * d3max);
     TE = std::max(4, std::min(64, TE / 4 * 4));
-    while ((size_t)(n * TE * d3max + n * n + TE * 16) * sizeof(float) > 200 * 1024 && TE > 4) TE -= 4;
+    auto smem_f = [&](int te) { return (size_t)(n * (te * d3max + 4) + n * n + te * 16) * sizeof(float); };
+    while (smem_f(TE) > 200 * 1024 && TE > 4) TE -= 4;
     te_f[L - 1] = TE;
     TpIo io{}; io.Mptr = Mptr; io.e_center = ws.e_center; io.geo = ws.geo; io.gamma = ws.gamma[L - 1];
     io.vprev = (L >= 2) ? ws.V[L - 2] : nullptr; io.winit = ws.winit_w1; io.ldwi = 2 * nsc; io.w = w;
     io.s = ws.s[L - 1]; io.vout = (L < NL) ? ws.V[L - 1] : nullptr;
     {
-      size_t smem = (size_t)(n * TE * d3max + n * n + TE * 16) * sizeof(float);
-      cudaFuncSetAttribute(k_tp_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
       dim3 grid((unsigned)((m_cap + TE - 1) / TE), (unsigned)(tp.has_lin ? tp.n_out : 1));
       prof_begin(m, st, KC_TP_FWD, tp_work(P, L, false));
-      k_tp_fwd<<<grid, TP_T, smem, st>>>(tp, io, TE);
+      launch_tp_fwd(m->tp_sig[L - 1], grid, smem_f(TE), st, tp, io, TE);
       prof_end(m, st);
     }
     m->launches += 2;
@@ -278,16 +305,15 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
       const int d3max = d3m[L - 1];
       const size_t per_edge = (size_t)n * (ly.in_dim + dsh) + 16;
       int TE = 32;
-      auto smem_of = [&](int te) { return (per_edge * te + 2 * (size_t)n * te * d3max + (size_t)n * n) * sizeof(float); };
+      auto smem_of = [&](int te) { return (per_edge * te + 2 * (size_t)n * (tp_ldr(te * d3max) + 4) + (size_t)n * n) * sizeof(float); };
       while (TE > 4 && smem_of(TE) > 200 * 1024) TE -= 4;
       if (smem_of(TE) > 227 * 1024) { m->err = "tensor-product backward tile does not fit in shared memory"; return ALLEGRO_ERR_UNSUPPORTED; }
       TpIo io{}; io.Mptr = Mptr; io.e_center = ws.e_center; io.geo = ws.geo; io.gamma = ws.gamma[L - 1];
       io.vprev = (L >= 2) ? ws.V[L - 2] : nullptr; io.winit = ws.winit_w1; io.ldwi = 2 * nsc; io.w = w;
       io.sbar = ws.sb; io.vbar = (L < NL) ? ws.vb[vcur] : nullptr; io.vbar_prev = ws.vb[vcur ^ 1]; io.ge = ws.ge;
       size_t smem = smem_of(TE);
-      cudaFuncSetAttribute(k_tp_bwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
       prof_begin(m, st, KC_TP_BWD, tp_work(P, L, true));
-      k_tp_bwd<<<(unsigned)((m_cap + TE - 1) / TE), TP_T, smem, st>>>(tp, io, TE, d3max);
+      launch_tp_bwd(m->tp_sig[L - 1], dim3((unsigned)((m_cap + TE - 1) / TE)), smem, st, tp, io, TE, d3max);
       prof_end(m, st);
       vcur ^= 1;
       m->launches += 1;

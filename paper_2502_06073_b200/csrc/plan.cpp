@@ -105,6 +105,18 @@ std::vector<double> coupling_tensor(int l1, int l2, int l3) {
   return C;
 }
 
+std::string layer_signature(const Layer& ly, int lmax) {
+  std::string s = "L" + std::to_string(lmax) + "|in";
+  for (const Irrep& a : ly.in_irreps) s += ":" + std::to_string(a.l) + (a.p > 0 ? "e" : "o");
+  s += "|out";
+  for (size_t o = 0; o < ly.out_irreps.size(); ++o)
+    s += ":" + std::to_string(ly.out_irreps[o].l) + (ly.out_irreps[o].p > 0 ? "e" : "o") + "@" + std::to_string(ly.out_off[o]);
+  s += "|p";
+  for (const Path& p : ly.paths)
+    s += ":" + std::to_string(p.ir1) + "," + std::to_string(p.l2) + "," + std::to_string(p.iro) + "," + std::to_string(p.pidx);
+  return s;
+}
+
 std::string build_plan(const allegro_hparams& hp, Plan* out) {
   Plan P;
   P.hp = hp;

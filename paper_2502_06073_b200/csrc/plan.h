@@ -68,6 +68,10 @@ struct Plan {
 // Returns "" on success, else an error message.  Does not touch CUDA.
 std::string build_plan(const allegro_hparams& hp, Plan* out);
 
+// Text key of one layer's tensor-product structure (irreps in/out, paths in order): two layers with the same key
+// run the same generated coupling code (gen_tp.cpp -> tp_gen.cuh).
+std::string layer_signature(const Layer& ly, int lmax);
+
 // Real coupling tensor for (l1,l2,l3) in the F3 basis, dense [2l1+1][2l2+1][2l3+1] (double).
 std::vector<double> coupling_tensor(int l1, int l2, int l3);
 

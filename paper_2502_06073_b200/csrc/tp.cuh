@@ -1,8 +1,11 @@
 // tp.cuh — F8/F9/F11 and B2/B5: the channel-wise Clebsch-Gordan tensor product V (x) Gamma of one layer, fused
 // with the channel-mixing linear W_lin (forward) / its transpose (backward), so that the per-path product T is
 // only ever held as a shared-memory tile ("64 tensor features with l=2 in full O(3) symmetry";
-// readings A8, A9, A12).  The sparse coupling tables (nonzeros grouped by output component) live in global
-// memory and are read through L1 by every thread in lock-step (uniform control flow).
+// readings A8, A9, A12).  The sparse coupling tensors are straight-line FMA code generated at build time
+// (gen_tp.cpp -> tp_gen.cuh), one kernel instantiation per layer signature: V, Gamma and T stay in registers.
+//
+// Layouts (channel fastest, so that a warp's loads/stores are contiguous):
+//   V[e][comp][c], Vbar[e][comp][c], GE[e][lm][c], Gamma[a][lm][c], winit/wenv/wbar[e][l*n + c], s[e][pidx*n + c].
 #pragma once
 #include <cuda_runtime.h>
 
@@ -10,6 +13,7 @@
 
 #include "device_math.cuh"
 #include "model.h"
+#include "tp_gen.cuh"
 
 namespace allegro {
 
@@ -18,9 +22,7 @@ constexpr int TP_T = 256;
 
 struct TpLayerDev {
   int n, lmax, dsh, in_dim, out_dim, n_paths, n_out, layer1, has_lin;
-  const int* path_tab;     // [n_paths][8]: in_off, d1, l2off, d2, iro, pidx, cg_begin, cg_end
-  const int* cg_idx;       // m1 | m2<<8 | m3<<16
-  const float* cg_val;
+  const int* path_tab;     // [n_paths][8]: in_off, d1, l2off, d2, iro, pidx, -, -
   int out_d3[TP_MAX_OUT], out_off[TP_MAX_OUT], out_np[TP_MAX_OUT];
   long long wlin[TP_MAX_OUT];   // blob offsets of W_lin^{(l,p)}  [n, np*n]
 };
@@ -29,34 +31,41 @@ struct TpIo {
   const int64_t* Mptr;
   const int* e_center;
   const float* geo;
-  const float* gamma;      // [atoms, n, dsh]
-  const float* vprev;      // [E, n, in_dim]      (layers >= 2)
-  const float* winit; int ldwi;   // [E, .] first n_sc columns = W_init x0   (layer 1)
+  const float* gamma;      // [atoms, dsh, n]
+  const float* vprev;      // [E, in_dim, n]      (layers >= 2)
+  const float* winit; int ldwi;   // [E, .] first n_sc columns = W_init x0, column l*n + c   (layer 1)
   const float* w;          // weight blob
   float* s;                // [E, n_sc]   scalars (forward)
-  float* vout;             // [E, n, out_dim]     (forward, has_lin)
+  float* vout;             // [E, out_dim, n]     (forward, has_lin)
   // backward
   const float* sbar;       // [E, n_sc]
-  const float* vbar;       // [E, n, out_dim]  adjoint of V^L (has_lin)
-  float* vbar_prev;        // [E, n, in_dim]
-  float* ge;               // [E, n, dsh]  per-edge contribution to Gammabar
+  const float* vbar;       // [E, out_dim, n]  adjoint of V^L (has_lin)
+  float* vbar_prev;        // [E, in_dim, n]
+  float* ge;               // [E, dsh, n]  per-edge contribution to Gammabar
 };
 
-// value of V^{L-1}[e, c, in_off + m1]
-__device__ __forceinline__ float tp_load_v(const TpLayerDev& ly, const TpIo& io, int64_t e, int c, int in_off, int d1, int m1,
-                                           const float* Ys_e) {
-  if (ly.layer1) {
-    const int l1 = (d1 - 1) >> 1;
-    return io.winit[e * io.ldwi + c * (ly.lmax + 1) + l1] * Ys_e[in_off + m1];   // V^0 = (W_init x0)_{c,l} Y_lm (F5); in_off = l^2
-  }
-  return io.vprev[(e * ly.n + c) * ly.in_dim + in_off + m1];
-}
+__host__ __device__ __forceinline__ int tp_ldr(int R) { return (R % 8 == 0) ? R + 4 : R; }
+__device__ __forceinline__ int l_of_lm(int k) { return (k >= 9) ? 3 : (k >= 4) ? 2 : (k >= 1) ? 1 : 0; }
 
-// ---------------------------------------------------------------------------------------------------------
-// forward: grid = (edge tiles, out irreps).  smem: Tt[n][R] | Ws[n][n] | Ys[TE][16]
-// ---------------------------------------------------------------------------------------------------------
+// accessor of V^{L-1}[e, c, k]: layer 1 forms V^0 = (W_init x0)_{c,l} Y_lm on the fly (F5)
+struct VAcc {
+  const float* base; int stride; const float* Y; bool layer1;
+  __device__ __forceinline__ float operator()(int k) const {
+    if (layer1) return base[l_of_lm(k) * stride] * Y[k];
+    return base[k * stride];
+  }
+};
+struct GAcc {
+  const float* base; int stride;
+  __device__ __forceinline__ float operator()(int k) const { return base[k * stride]; }
+};
+
 constexpr int TP_MAXMT = 4;   // 4x4 micro-tiles per thread
 
+// ---------------------------------------------------------------------------------------------------------
+// forward: grid = (edge tiles, out irreps).  smem: Tt[n][ldR] | Ws[n][n] | Ys[TE][16]
+// ---------------------------------------------------------------------------------------------------------
+template <int SIG>
 __global__ void __launch_bounds__(TP_T) k_tp_fwd(TpLayerDev ly, TpIo io, int TE) {
   extern __shared__ __align__(16) float sm[];
   const int64_t M = *io.Mptr;
@@ -64,12 +73,13 @@ __global__ void __launch_bounds__(TP_T) k_tp_fwd(TpLayerDev ly, TpIo io, int TE)
   if (e0 >= M) return;
   const int o = blockIdx.y;
   const int n = ly.n, d3 = ly.out_d3[o];
-  const int R = TE * d3;                       // TE is a multiple of 4
-  float* Tt = sm;                              // [n][R]
-  float* Ws = Tt + n * R;                      // [n][n]  Ws[c][c'] = W[c', pidx n + c]
+  const int R = TE * d3, ldR = tp_ldr(R);    // TE is a multiple of 4
+  float* Tt = sm;                              // [n][ldR]
+  float* Ws = Tt + n * ldR;                    // [n][n]  Ws[c][c'] = W[c', pidx n + c]
   float* Ys = Ws + n * n;                      // [TE][16]
   const int tid = threadIdx.x;
   const int ne = (int)min((int64_t)TE, M - e0);
+  const int nsc = n * (ly.lmax + 1);
   for (int t = tid; t < TE; t += TP_T) {
     float* y = Ys + t * 16;
     if (t < ne) { const float* gq = io.geo + (e0 + t) * GEO_W; sph_harm_rt(ly.lmax, gq[0], gq[1], gq[2], y); }
@@ -89,25 +99,18 @@ __global__ void __launch_bounds__(TP_T) k_tp_fwd(TpLayerDev ly, TpIo io, int TE)
   for (int p = 0; p < ly.n_paths; ++p) {
     const int* pt = ly.path_tab + p * 8;
     if (pt[4] != o) continue;
-    const int in_off = pt[0], d1 = pt[1], l2off = pt[2], pidx = pt[5], cb = pt[6], ce = pt[7];
-    // T_p[e, c, m3] for the tile
+    const int pidx = pt[5];
+    // T_p[e, c, m3] for the tile: one (edge, channel) pair per thread and iteration, channel fastest
     for (int idx = tid; idx < TE * n; idx += TP_T) {
-      const int el = idx % TE, c = idx / TE;
-      float* dst = Tt + c * R + el * d3;
+      const int c = idx % n, el = idx / n;
+      float* dst = Tt + c * ldR + el * d3;
       if (el >= ne) { for (int m = 0; m < d3; ++m) dst[m] = 0.f; continue; }
       const int64_t e = e0 + el;
-      const float* G = io.gamma + ((int64_t)io.e_center[e] * n + c) * ly.dsh + l2off;
-      const float* Ye = Ys + el * 16;
-      float a = 0.f; int cur = -1;
-      for (int m = 0; m < d3; ++m) dst[m] = 0.f;
-      for (int q = cb; q < ce; ++q) {
-        const int pk = ly.cg_idx[q];
-        const int m1 = pk & 255, m2 = (pk >> 8) & 255, m3 = pk >> 16;
-        if (m3 != cur) { if (cur >= 0) dst[cur] = a; cur = m3; a = 0.f; }
-        a = fmaf(ly.cg_val[q] * tp_load_v(ly, io, e, c, in_off, d1, m1, Ye), G[m2], a);
-      }
-      if (cur >= 0) dst[cur] = a;
-      if (o == 0) io.s[e * (n * (ly.lmax + 1)) + pidx * n + c] = dst[0];   // F9: path-major, then channel
+      VAcc V{ly.layer1 ? io.winit + e * io.ldwi + c : io.vprev + e * ly.in_dim * n + c, n, Ys + el * 16, ly.layer1 != 0};
+      GAcc G{io.gamma + (int64_t)io.e_center[e] * ly.dsh * n + c, n};
+      float t0 = 0.f;
+      tpgen::tp_path_fwd<SIG>(p, V, G, [&](int m, float v) { dst[m] = v; if (m == 0) t0 = v; });
+      if (o == 0) io.s[e * nsc + pidx * n + c] = t0;   // F9: path-major, then channel
     }
     if (lin) {
       for (int idx = tid; idx < n * n; idx += TP_T) {
@@ -123,7 +126,7 @@ __global__ void __launch_bounds__(TP_T) k_tp_fwd(TpLayerDev ly, TpIo io, int TE)
         if (mt < nmt) {
           const int tr = mt % ntr, tc = mt / ntr;
           for (int k = 0; k < n; ++k) {
-            const float4 av = *reinterpret_cast<const float4*>(Tt + k * R + tr * 4);
+            const float4 av = *reinterpret_cast<const float4*>(Tt + k * ldR + tr * 4);
             const float4 bv = *reinterpret_cast<const float4*>(Ws + k * n + tc * 4);
             const float a4[4] = {av.x, av.y, av.z, av.w}, b4[4] = {bv.x, bv.y, bv.z, bv.w};
 #pragma unroll
@@ -146,10 +149,9 @@ __global__ void __launch_bounds__(TP_T) k_tp_fwd(TpLayerDev ly, TpIo io, int TE)
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
           const int r = tr * 4 + i, el = r / d3, m = r - el * d3;
-          if (el < ne) {
-#pragma unroll
-            for (int j = 0; j < 4; ++j) io.vout[((e0 + el) * n + tc * 4 + j) * ly.out_dim + ooff + m] = acc[q][i][j];
-          }
+          if (el < ne)
+            *reinterpret_cast<float4*>(io.vout + ((e0 + el) * ly.out_dim + ooff + m) * n + tc * 4) =
+                make_float4(acc[q][i][0], acc[q][i][1], acc[q][i][2], acc[q][i][3]);
         }
       }
     }
@@ -158,41 +160,44 @@ __global__ void __launch_bounds__(TP_T) k_tp_fwd(TpLayerDev ly, TpIo io, int TE)
 
 // ---------------------------------------------------------------------------------------------------------
 // backward: one block per TE edges, all out irreps and paths.
-// smem: VB[TE][n][in_dim] | GE[TE][n][dsh] | At[n][Rmax] | Tt[n][Rmax] | Ws[n][n] | Ys[TE][16]
+// smem: VB[TE][in_dim][n] | GE[TE][dsh][n] | At[n][ldRmax] | Tt[n][ldRmax] | Ws[n][n] | Ys[TE][16]
 // ---------------------------------------------------------------------------------------------------------
+template <int SIG>
 __global__ void __launch_bounds__(TP_T) k_tp_bwd(TpLayerDev ly, TpIo io, int TE, int d3max) {
   extern __shared__ __align__(16) float sm[];
   const int64_t M = *io.Mptr;
   const int64_t e0 = (int64_t)blockIdx.x * TE;
   if (e0 >= M) return;
-  const int n = ly.n, Rmax = TE * d3max;
+  const int n = ly.n, ldRmax = tp_ldr(TE * d3max) + 4;
   float* VB = sm;
   float* GE = VB + TE * n * ly.in_dim;
   float* At = GE + TE * n * ly.dsh;
-  float* Tt = At + n * Rmax;
-  float* Ws = Tt + n * Rmax;
+  float* Tt = At + n * ldRmax;
+  float* Ws = Tt + n * ldRmax;
   float* Ys = Ws + n * n;
   const int tid = threadIdx.x;
   const int ne = (int)min((int64_t)TE, M - e0);
+  const int nsc = n * (ly.lmax + 1);
   for (int t = tid; t < TE; t += TP_T)
     if (t < ne) { const float* gq = io.geo + (e0 + t) * GEO_W; sph_harm_rt(ly.lmax, gq[0], gq[1], gq[2], Ys + t * 16); }
   for (int idx = tid; idx < TE * n * (ly.in_dim + ly.dsh); idx += TP_T) VB[idx] = 0.f;   // VB and GE are adjacent
   __syncthreads();
   for (int o = 0; o < ly.n_out; ++o) {
-    const int d3 = ly.out_d3[o], R = TE * d3;
+    const int d3 = ly.out_d3[o], R = TE * d3, ldR = tp_ldr(R);
     const bool lin = ly.has_lin && ly.out_off[o] >= 0;
+    if (!lin && o != 0) continue;
     const float* Wo = lin ? io.w + ly.wlin[o] : nullptr;
     const int ldw = ly.out_np[o] * n;
-    if (lin) {   // At[c'][el*d3+m] = Vbar^L[e, c', o, m]
+    if (lin) {   // At[c'][el*d3+m] = Vbar^L[e, o, m, c']
       for (int idx = tid; idx < TE * n * d3; idx += TP_T) {
-        const int m = idx % d3, t2 = idx / d3, cp = t2 % n, el = t2 / n;
-        At[cp * R + el * d3 + m] = (el < ne) ? io.vbar[((e0 + el) * n + cp) * ly.out_dim + ly.out_off[o] + m] : 0.f;
+        const int cp = idx % n, t2 = idx / n, m = t2 % d3, el = t2 / d3;
+        At[cp * ldR + el * d3 + m] = (el < ne) ? io.vbar[((e0 + el) * ly.out_dim + ly.out_off[o] + m) * n + cp] : 0.f;
       }
     }
     for (int p = 0; p < ly.n_paths; ++p) {
       const int* pt = ly.path_tab + p * 8;
       if (pt[4] != o) continue;
-      const int in_off = pt[0], d1 = pt[1], l2off = pt[2], pidx = pt[5], cb = pt[6], ce = pt[7];
+      const int pidx = pt[5];
       if (lin) {
         for (int idx = tid; idx < n * n; idx += TP_T) {   // Ws[c'][c] = W[c', pidx n + c]  (B2)
           const int cp = idx / n, c = idx - cp * n;
@@ -211,7 +216,7 @@ __global__ void __launch_bounds__(TP_T) k_tp_bwd(TpLayerDev ly, TpIo io, int TE,
           for (int j = 0; j < 4; ++j) a[i][j] = 0.f;
         if (lin) {
           for (int k = 0; k < n; ++k) {
-            const float4 av = *reinterpret_cast<const float4*>(At + k * R + tr * 4);
+            const float4 av = *reinterpret_cast<const float4*>(At + k * ldR + tr * 4);
             const float4 bv = *reinterpret_cast<const float4*>(Ws + k * n + tc * 4);
             const float a4[4] = {av.x, av.y, av.z, av.w}, b4[4] = {bv.x, bv.y, bv.z, bv.w};
 #pragma unroll
@@ -221,33 +226,32 @@ __global__ void __launch_bounds__(TP_T) k_tp_bwd(TpLayerDev ly, TpIo io, int TE,
           }
         }
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
-#pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            const int r = tr * 4 + i, c = tc * 4 + j;
-            float v = a[i][j];
-            if (o == 0 && r < ne) v += io.sbar[(e0 + r) * (n * (ly.lmax + 1)) + pidx * n + c];   // d3 == 1: r == el
-            Tt[c * R + r] = v;
+        for (int j = 0; j < 4; ++j) {
+          const int c = tc * 4 + j;
+          float4 v = make_float4(a[0][j], a[1][j], a[2][j], a[3][j]);
+          if (o == 0) {   // d3 == 1: row r == el
+            const int r = tr * 4;
+            if (r < ne) v.x += io.sbar[(e0 + r) * nsc + pidx * n + c];
+            if (r + 1 < ne) v.y += io.sbar[(e0 + r + 1) * nsc + pidx * n + c];
+            if (r + 2 < ne) v.z += io.sbar[(e0 + r + 2) * nsc + pidx * n + c];
+            if (r + 3 < ne) v.w += io.sbar[(e0 + r + 3) * nsc + pidx * n + c];
           }
+          *reinterpret_cast<float4*>(Tt + c * ldR + tr * 4) = v;
+        }
       }
       __syncthreads();
       // B5: Vbar^{L-1}[m1] += C Tbar[m3] Gamma[m2];  GE[m2] += C Tbar[m3] V[m1]
       for (int idx = tid; idx < TE * n; idx += TP_T) {
-        const int el = idx % TE, c = idx / TE;
+        const int c = idx % n, el = idx / n;
         if (el >= ne) continue;
         const int64_t e = e0 + el;
-        const float* G = io.gamma + ((int64_t)io.e_center[e] * n + c) * ly.dsh + l2off;
-        const float* Ye = Ys + el * 16;
-        const float* tb = Tt + c * R + el * d3;
-        float* vb = VB + (el * n + c) * ly.in_dim + in_off;
-        float* gb = GE + (el * n + c) * ly.dsh + l2off;
-        for (int q = cb; q < ce; ++q) {
-          const int pk = ly.cg_idx[q];
-          const int m1 = pk & 255, m2 = (pk >> 8) & 255, m3 = pk >> 16;
-          const float ct = ly.cg_val[q] * tb[m3];
-          vb[m1] = fmaf(ct, G[m2], vb[m1]);
-          gb[m2] = fmaf(ct, tp_load_v(ly, io, e, c, in_off, d1, m1, Ye), gb[m2]);
-        }
+        VAcc V{ly.layer1 ? io.winit + e * io.ldwi + c : io.vprev + e * ly.in_dim * n + c, n, Ys + el * 16, ly.layer1 != 0};
+        GAcc G{io.gamma + (int64_t)io.e_center[e] * ly.dsh * n + c, n};
+        const float* tb = Tt + c * ldR + el * d3;
+        float* vb = VB + el * ly.in_dim * n + c;
+        float* gb = GE + el * ly.dsh * n + c;
+        tpgen::tp_path_bwd<SIG>(p, V, G, [&](int m) { return tb[m]; }, [&](int k, float v) { vb[k * n] += v; },
+                                [&](int k, float v) { gb[k * n] += v; });
       }
       __syncthreads();
     }
