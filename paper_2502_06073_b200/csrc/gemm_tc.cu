@@ -151,41 +151,51 @@ __global__ void __launch_bounds__(TC_T) k_gemm_tc(GemmArgs a, const float* __res
   if (a.pro == PRO_SCALE_U && arow_ok) ascale = a.c_new * a.geo[arow * GEO_W + 4];
   const int off_row = (r >> 3) * (TC_KC / 4) * 32 + (r & 7) * 4;   // floats: (row/8)*SBO + (row%8)*16 B
 
-  for (int c = 0; c < nchunks; ++c) {
-    const int b = c & 1;
-    if (c >= 2) mbar_wait(&mbar_mma[b], (uint32_t)(((c >> 1) - 1) & 1));   // MMAs of slice c-2 have drained stage b
-    uint8_t* st = smem_raw + (size_t)b * stage_bytes;
-    float* Ahi = reinterpret_cast<float*>(st);
-    float* Alo = reinterpret_cast<float*>(st + a_bytes);
-    float* Bhi = reinterpret_cast<float*>(st + 2 * a_bytes);
-    if (tid == 0) bulk_g2s(Bhi, Bt + (int64_t)c * (2 * Nt * TC_KC), 2 * b_bytes, &mbar_b[b]);
-    const int k0 = c * TC_KC;
+  // raw A values of one 16-deep slice (this thread: row r, k-quads 2*qh and 2*qh+1), no prologue applied yet
+  auto load_slice = [&](int c, float (&v)[2][4]) {
 #pragma unroll
     for (int qq = 0; qq < 2; ++qq) {
-      const int q = qh * 2 + qq;
-      const int kk = k0 + q * 4;
-      float v[4] = {0.f, 0.f, 0.f, 0.f};
+      const int kk = c * TC_KC + (qh * 2 + qq) * 4;
+#pragma unroll
+      for (int e = 0; e < 4; ++e) v[qq][e] = 0.f;
       if (arow_ok && kk < K) {
         const float* src; int kl, kmax;
         if (kk < a.K0) { src = a.A0 + arow * a.lda0; kl = kk; kmax = a.K0; }
         else { src = a.A1 + arow * a.lda1; kl = kk - a.K0; kmax = a.K1; }
         if (kl + 3 < kmax && ((((uintptr_t)(src + kl)) & 15) == 0)) {
           const float4 t = *reinterpret_cast<const float4*>(src + kl);
-          v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+          v[qq][0] = t.x; v[qq][1] = t.y; v[qq][2] = t.z; v[qq][3] = t.w;
         } else {
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
             const int kq = kk + e;
-            if (kq < K) v[e] = (kq < a.K0) ? a.A0[arow * a.lda0 + kq] : a.A1[arow * a.lda1 + (kq - a.K0)];
+            if (kq < K) v[qq][e] = (kq < a.K0) ? a.A0[arow * a.lda0 + kq] : a.A1[arow * a.lda1 + (kq - a.K0)];
           }
         }
-        if (a.pro == PRO_SILU) {
+      }
+    }
+  };
+  float vcur[2][4], vnext[2][4];
+  load_slice(0, vcur);
+  for (int c = 0; c < nchunks; ++c) {
+    const int b = c & 1;
+    if (c + 1 < nchunks) load_slice(c + 1, vnext);                        // in flight while slice c is staged and issued
+    if (c >= 2) mbar_wait(&mbar_mma[b], (uint32_t)(((c >> 1) - 1) & 1));   // MMAs of slice c-2 have drained stage b
+    uint8_t* st = smem_raw + (size_t)b * stage_bytes;
+    float* Ahi = reinterpret_cast<float*>(st);
+    float* Alo = reinterpret_cast<float*>(st + a_bytes);
+    float* Bhi = reinterpret_cast<float*>(st + 2 * a_bytes);
+    if (tid == 0) bulk_g2s(Bhi, Bt + (int64_t)c * (2 * Nt * TC_KC), 2 * b_bytes, &mbar_b[b]);
 #pragma unroll
-          for (int e = 0; e < 4; ++e) v[e] = silu_f(v[e]);
-        } else if (a.pro == PRO_SCALE_U) {
+    for (int qq = 0; qq < 2; ++qq) {
+      const int q = qh * 2 + qq;
+      float v[4] = {vcur[qq][0], vcur[qq][1], vcur[qq][2], vcur[qq][3]};
+      if (a.pro == PRO_SILU) {
 #pragma unroll
-          for (int e = 0; e < 4; ++e) v[e] *= ascale;
-        }
+        for (int e = 0; e < 4; ++e) v[e] = silu_f(v[e]);
+      } else if (a.pro == PRO_SCALE_U) {
+#pragma unroll
+        for (int e = 0; e < 4; ++e) v[e] *= ascale;
       }
       float4 hi, lo;
       hi.x = tf32_rna(v[0]); hi.y = tf32_rna(v[1]); hi.z = tf32_rna(v[2]); hi.w = tf32_rna(v[3]);
@@ -193,6 +203,10 @@ __global__ void __launch_bounds__(TC_T) k_gemm_tc(GemmArgs a, const float* __res
       *reinterpret_cast<float4*>(Ahi + off_row + q * 32) = hi;
       *reinterpret_cast<float4*>(Alo + off_row + q * 32) = lo;
     }
+#pragma unroll
+    for (int qq = 0; qq < 2; ++qq)
+#pragma unroll
+      for (int e = 0; e < 4; ++e) vcur[qq][e] = vnext[qq][e];
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy smem writes -> visible to the tensor core
     __syncthreads();
     if (tid == 0) {

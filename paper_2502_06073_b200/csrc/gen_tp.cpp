@@ -125,7 +125,25 @@ int main(int argc, char** argv) {
   fprintf(f, "constexpr int N_SIGS = %zu;\n", sigs.size());
   fprintf(f, "static const char* const SIG_STR[N_SIGS] = {\n");
   for (const std::string& s : sigs) fprintf(f, "  \"%s\",\n", s.c_str());
-  fprintf(f, "};\n\n#ifdef __CUDACC__\n");
+  fprintf(f, "};\n");
+  fprintf(f, "template <int SIG> struct SigDims;\n");
+  for (size_t i = 0; i < sigs.size(); ++i) {
+    const Layer& ly = layers[i];
+    int lmax = sigs[i][1] - '0';
+    auto arr = [&](const char* name, const std::vector<int>& v) {
+      fprintf(f, "  static constexpr __host__ __device__ int %s(int i) { constexpr int t[] = {", name);
+      for (size_t k = 0; k < v.size(); ++k) fprintf(f, "%s%d", k ? ", " : "", v[k]);
+      fprintf(f, "}; return t[i]; }\n");
+    };
+    std::vector<int> piro, ppidx, od3, onp, ooff;
+    for (const Path& pa : ly.paths) { piro.push_back(pa.iro); ppidx.push_back(pa.pidx); }
+    for (size_t o = 0; o < ly.out_irreps.size(); ++o) { od3.push_back(2 * ly.out_irreps[o].l + 1); onp.push_back(ly.out_npaths[o]); ooff.push_back(ly.out_off[o]); }
+    fprintf(f, "template <> struct SigDims<%zu> {\n  static constexpr int IN_DIM = %d, DSH = %d, LMAX = %d, NPATH = %zu, NOUT = %zu, OUT_DIM = %d;\n", i,
+            ly.in_dim, (lmax + 1) * (lmax + 1), lmax, ly.paths.size(), ly.out_irreps.size(), ly.out_dim);
+    arr("p_iro", piro); arr("p_pidx", ppidx); arr("o_d3", od3); arr("o_np", onp); arr("o_off", ooff);
+    fprintf(f, "};\n");
+  }
+  fprintf(f, "\n#ifdef __CUDACC__\n");
   for (size_t i = 0; i < sigs.size(); ++i) emit_layer(f, (int)i, layers[i]);
   fprintf(f, "template <int SIG, class VA, class GA, class TA>\n__device__ __forceinline__ void tp_path_fwd(int p, VA V, GA G, TA T) {\n");
   for (size_t i = 0; i < sigs.size(); ++i) fprintf(f, "  if constexpr (SIG == %zu) tp_path_fwd_%zu(p, V, G, T);\n", i, i);

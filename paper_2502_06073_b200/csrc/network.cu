@@ -111,34 +111,6 @@ static double tp_work(const Plan& P, int L, bool backward) {
   return f;
 }
 
-// launch the generated instantiation of the tensor-product kernels for layer signature `sig`
-static void launch_tp_fwd(int sig, dim3 grid, size_t smem, cudaStream_t st, const TpLayerDev& tp, const TpIo& io, int TE) {
-  static bool attr[tpgen::N_SIGS] = {false};
-  switch (sig) {
-#define X(I)                                                                                                        \
-  case I:                                                                                                           \
-    if (!attr[I]) { cudaFuncSetAttribute(k_tp_fwd<I>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); attr[I] = true; } \
-    k_tp_fwd<I><<<grid, TP_T, smem, st>>>(tp, io, TE);                                                              \
-    break;
-    TPGEN_FOR_EACH_SIG(X)
-#undef X
-    default: break;
-  }
-}
-static void launch_tp_bwd(int sig, dim3 grid, size_t smem, cudaStream_t st, const TpLayerDev& tp, const TpIo& io, int TE, int d3max) {
-  static bool attr[tpgen::N_SIGS] = {false};
-  switch (sig) {
-#define X(I)                                                                                                        \
-  case I:                                                                                                           \
-    if (!attr[I]) { cudaFuncSetAttribute(k_tp_bwd<I>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024); attr[I] = true; } \
-    k_tp_bwd<I><<<grid, TP_T, smem, st>>>(tp, io, TE, d3max);                                                       \
-    break;
-    TPGEN_FOR_EACH_SIG(X)
-#undef X
-    default: break;
-  }
-}
-
 static TpLayerDev make_tp(const Model* m, int L) {
   const Plan& P = m->plan;
   const Layer& ly = P.layers[L - 1];
@@ -225,10 +197,15 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
     int d3max = 1;
     for (int o = 0; o < tp.n_out; ++o) if (tp.has_lin || o == 0) d3max = std::max(d3max, tp.out_d3[o]);
     d3m[L - 1] = d3max;
-    int TE = (16 * TP_T * TP_MAXMT) / (n * d3max);
-    TE = std::max(4, std::min(64, TE / 4 * 4));
-    auto smem_f = [&](int te) { return (size_t)(n * (te * d3max + 4) + n * n + te * 16) * sizeof(float); };
-    while (smem_f(TE) > 200 * 1024 && TE > 4) TE -= 4;
+    int npmax = 1;
+    for (int o = 0; o < tp.n_out; ++o) if (tp.has_lin || o == 0) npmax = std::max(npmax, tp.out_np[o]);
+    const size_t budget = (n <= 32 ? 56 : 100) * 1024;
+    int TE = 32;
+    while (TE > 4 && TE * d3max * n > 16 * TP_T * TP_MAXMT) TE >>= 1;
+    auto smem_f = [&](int te, int pc) { return (size_t)(pc * n * (tp_ldr(te * d3max) + n) + te * 16) * sizeof(float); };
+    int PC = npmax;
+    while (PC > 1 && smem_f(TE, PC) > budget) --PC;
+    while (TE > 4 && smem_f(TE, PC) > 200 * 1024) TE >>= 1;
     te_f[L - 1] = TE;
     TpIo io{}; io.Mptr = Mptr; io.e_center = ws.e_center; io.geo = ws.geo; io.gamma = ws.gamma[L - 1];
     io.vprev = (L >= 2) ? ws.V[L - 2] : nullptr; io.winit = ws.winit_w1; io.ldwi = 2 * nsc; io.w = w;
@@ -236,7 +213,14 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
     {
       dim3 grid((unsigned)((m_cap + TE - 1) / TE), (unsigned)(tp.has_lin ? tp.n_out : 1));
       prof_begin(m, st, KC_TP_FWD, tp_work(P, L, false));
-      launch_tp_fwd(m->tp_sig[L - 1], grid, smem_f(TE), st, tp, io, TE);
+      if (tp3_supported(tp) && m->use_tp3) {
+        const size_t sm3 = tp3_smem_bytes(tp, false);
+        const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(3, (200 * 1024) / std::max<size_t>(sm3, 1)));
+        const int64_t nsub = (m_cap + 256 / n - 1) / (256 / n);
+        launch_tp3(m->tp_sig[L - 1], false, (int)std::min<int64_t>(nsub, (int64_t)m->num_sms * per_sm), st, tp, io);
+      } else {
+        launch_tp_fwd(m->tp_sig[L - 1], grid, smem_f(TE, PC), st, tp, io, TE, PC);
+      }
       prof_end(m, st);
     }
     m->launches += 2;
@@ -304,16 +288,31 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
     {
       const int d3max = d3m[L - 1];
       const size_t per_edge = (size_t)n * (ly.in_dim + dsh) + 16;
+      int npmax = 1;
+      for (int o = 0; o < tp.n_out; ++o) if (tp.has_lin || o == 0) npmax = std::max(npmax, tp.out_np[o]);
+      const size_t budget = (n <= 32 ? 56 : 110) * 1024;
+      auto smem_of = [&](int te, int pc) {
+        return (per_edge * te + (size_t)(1 + pc) * n * (tp_ldr(te * d3max) + 4) + (size_t)pc * n * n) * sizeof(float);
+      };
       int TE = 32;
-      auto smem_of = [&](int te) { return (per_edge * te + 2 * (size_t)n * (tp_ldr(te * d3max) + 4) + (size_t)n * n) * sizeof(float); };
-      while (TE > 4 && smem_of(TE) > 200 * 1024) TE -= 4;
-      if (smem_of(TE) > 227 * 1024) { m->err = "tensor-product backward tile does not fit in shared memory"; return ALLEGRO_ERR_UNSUPPORTED; }
+      while (TE > 4 && smem_of(TE, 1) > budget / 2) TE >>= 1;
+      int PC = npmax;
+      while (PC > 1 && smem_of(TE, PC) > budget) --PC;
+      if (smem_of(TE, PC) > 220 * 1024) { m->err = "tensor-product backward tile does not fit in shared memory"; return ALLEGRO_ERR_UNSUPPORTED; }
       TpIo io{}; io.Mptr = Mptr; io.e_center = ws.e_center; io.geo = ws.geo; io.gamma = ws.gamma[L - 1];
       io.vprev = (L >= 2) ? ws.V[L - 2] : nullptr; io.winit = ws.winit_w1; io.ldwi = 2 * nsc; io.w = w;
       io.sbar = ws.sb; io.vbar = (L < NL) ? ws.vb[vcur] : nullptr; io.vbar_prev = ws.vb[vcur ^ 1]; io.ge = ws.ge;
-      size_t smem = smem_of(TE);
+      io.wbar_init = ws.wb; io.ldwb = 2 * nsc; io.ybar = ws.yb;   // layer 1: B8 applied inside the kernel
+      size_t smem = smem_of(TE, PC);
       prof_begin(m, st, KC_TP_BWD, tp_work(P, L, true));
-      launch_tp_bwd(m->tp_sig[L - 1], dim3((unsigned)((m_cap + TE - 1) / TE)), smem, st, tp, io, TE, d3max);
+      if (tp3_supported(tp) && m->use_tp3) {
+        const size_t sm3 = tp3_smem_bytes(tp, true);
+        const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(2, (200 * 1024) / std::max<size_t>(sm3, 1)));
+        const int64_t nsub = (m_cap + 256 / n - 1) / (256 / n);
+        launch_tp3(m->tp_sig[L - 1], true, (int)std::min<int64_t>(nsub, (int64_t)m->num_sms * per_sm), st, tp, io);
+      } else {
+        launch_tp_bwd(m->tp_sig[L - 1], dim3((unsigned)((m_cap + TE - 1) / TE)), smem, st, tp, io, TE, d3max, PC);
+      }
       prof_end(m, st);
       vcur ^= 1;
       m->launches += 1;
@@ -333,10 +332,7 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
       launch_gemm(m, g, m_cap, st);
     }
   }
-  // B8: adjoint of V^0, then [W_init; W_env^1]^T [wbar_init; wbar^1] in one GEMM (B7 of layer 1 + B8)
-  prof_begin(m, st, KC_EDGE_MISC, 0);
-  k_init_bwd<<<gridWE, T, 0, st>>>(Mptr, ws.geo, ws.vb[vcur], ws.winit_w1, 2 * nsc, n, hp.lmax, ws.wb, 2 * nsc, ws.yb);
-  prof_end(m, st);
+  // [W_init; W_env^1]^T [wbar_init; wbar^1] in one GEMM (B7 of layer 1 + B8; wbar_init comes from k_tp_bwd of layer 1)
   g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo; g.wtrans = 1;
   g.A0 = ws.wb; g.lda0 = g.K0 = 2 * nsc; g.W = w + P.w_init; g.ldw = D; g.N = D; g.C = ws.xb[xcur]; g.ldc = D; g.epi = EPI_ACCUM;
   launch_gemm(m, g, m_cap, st);
@@ -344,7 +340,7 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
   prof_begin(m, st, KC_EDGE_MISC, 0);
   k_rowdot<<<gridWE, T, 0, st>>>(Mptr, ws.xb[xcur], ws.y0, D, 1.0f, 1, ws.ub);
   prof_end(m, st);
-  m->launches += 2;
+  m->launches += 1;
   {
     const float* cur = ws.xb[xcur];
     int zc = 0;

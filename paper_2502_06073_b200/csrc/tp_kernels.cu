@@ -1,0 +1,75 @@
+// tp_kernels.cu — instantiations of the generated tensor-product kernels (tp.cuh, tp3.cuh) and their launchers, in a
+// translation unit of their own: one instantiation per layer signature of tp_gen.cuh.
+#include "tp3.cuh"
+
+namespace allegro {
+
+// launch the generated instantiation of the tensor-product kernels for layer signature `sig`
+void launch_tp_fwd(int sig, dim3 grid, size_t smem, cudaStream_t st, const TpLayerDev& tp, const TpIo& io, int TE, int PC) {
+  static bool attr[tpgen::N_SIGS] = {false};
+  switch (sig) {
+#define X(I)                                                                                                        \
+  case I:                                                                                                           \
+    if (!attr[I]) { cudaFuncSetAttribute(k_tp_fwd<I>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); attr[I] = true; } \
+    k_tp_fwd<I><<<grid, TP_T, smem, st>>>(tp, io, TE, PC);                                                            \
+    break;
+    TPGEN_FOR_EACH_SIG(X)
+#undef X
+    default: break;
+  }
+}
+void launch_tp_bwd(int sig, dim3 grid, size_t smem, cudaStream_t st, const TpLayerDev& tp, const TpIo& io, int TE, int d3max, int PC) {
+  static bool attr[tpgen::N_SIGS] = {false};
+  switch (sig) {
+#define X(I)                                                                                                        \
+  case I:                                                                                                           \
+    if (!attr[I]) { cudaFuncSetAttribute(k_tp_bwd<I>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024); attr[I] = true; } \
+    k_tp_bwd<I><<<grid, TP_T, smem, st>>>(tp, io, TE, d3max, PC);                                                     \
+    break;
+    TPGEN_FOR_EACH_SIG(X)
+#undef X
+    default: break;
+  }
+}
+
+
+// shared-memory bytes of the few-channel kernels (tp3.cuh); 0 when the layer has no channel mixing
+size_t tp3_smem_bytes(const TpLayerDev& tp, bool backward) {
+  if (!tp.has_lin) return 0;
+  const int n = tp.n, TE = 256 / n;
+  size_t f = 0;
+  for (int o = 0; o < tp.n_out; ++o) {
+    if (tp.out_off[o] < 0) continue;
+    const size_t K = (size_t)tp.out_np[o] * n, rows = tp3_round16(TE * tp.out_d3[o]);
+    f += backward ? 2 * n * (K + 8) + rows * (n + 4) + rows * (K + 4) : 2 * K * (n + 8) + rows * (K + 4);
+  }
+  return f * sizeof(float);
+}
+
+bool tp3_supported(const TpLayerDev& tp) {
+  const int n = tp.n;
+  if (!(n == 8 || n == 16 || n == 32) || tp.n_out > TP3_MAXO) return false;
+  return tp3_smem_bytes(tp, true) <= 200 * 1024 && tp3_smem_bytes(tp, false) <= 200 * 1024;
+}
+
+void launch_tp3(int sig, bool backward, int grid, cudaStream_t st, const TpLayerDev& tp, const TpIo& io) {
+  static bool attr_f[tpgen::N_SIGS] = {false}, attr_b[tpgen::N_SIGS] = {false};
+  const size_t smem = tp3_smem_bytes(tp, backward);
+  switch (sig) {
+#define X(I)                                                                                                         \
+  case I:                                                                                                            \
+    if (!backward) {                                                                                                 \
+      if (!attr_f[I]) { cudaFuncSetAttribute(k_tp_fwd3<I>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); attr_f[I] = true; } \
+      k_tp_fwd3<I><<<grid, 256, smem, st>>>(tp, io);                                                                 \
+    } else {                                                                                                         \
+      if (!attr_b[I]) { cudaFuncSetAttribute(k_tp_bwd3<I>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); attr_b[I] = true; } \
+      k_tp_bwd3<I><<<grid, 256, smem, st>>>(tp, io);                                                                 \
+    }                                                                                                                \
+    break;
+    TPGEN_FOR_EACH_SIG(X)
+#undef X
+    default: break;
+  }
+}
+
+}  // namespace allegro
