@@ -142,6 +142,7 @@ int allegro_create(const float* weights_host, size_t n_weights, const allegro_hp
   }
   cudaGetDevice(&m->device);
   { const char* g = std::getenv("ALLEGRO_GEMM"); m->use_tc = !(g && std::string(g) == "fp32"); }
+  { const char* g = std::getenv("ALLEGRO_CHAIN"); m->use_chain = !(g && std::string(g) == "0"); }
   { const char* g = std::getenv("ALLEGRO_TP"); m->use_tp3 = !(g && std::string(g) == "generic"); }
   cudaDeviceGetAttribute(&m->num_sms, cudaDevAttrMultiProcessorCount, m->device);
   auto fail = [&](int rc, const std::string& msg) { g_create_err = msg; allegro_destroy(m); return rc; };

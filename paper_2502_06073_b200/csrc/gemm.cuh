@@ -53,12 +53,14 @@ __device__ __forceinline__ void gemm_epi(const GemmArgs& a, int64_t row, int n, 
   }
 }
 
-// four consecutive output columns n..n+3 (n % 4 == 0, all < N, every leading dimension a multiple of 4)
-__device__ __forceinline__ void gemm_epi4(const GemmArgs& a, int64_t row, int n, float4 v, float u, int zi, int zj) {
+// four consecutive output columns n..n+3 (n % 4 == 0, all < N, every leading dimension a multiple of 4).
+// Returns the value a following chained stage consumes (gemm_chain.cu): the stored pre-activation for STORE / GATHER2,
+// x = u v for Y_X, the new latent for RESIDUAL, v silu'(z) for DSILU, the accumulated sum for ACCUM.
+__device__ __forceinline__ float4 gemm_epi4(const GemmArgs& a, int64_t row, int n, float4 v, float u, int zi, int zj) {
   auto ld4 = [](const float* p) { return *reinterpret_cast<const float4*>(p); };
   auto st4 = [](float* p, float4 x) { *reinterpret_cast<float4*>(p) = x; };
   switch (a.epi) {
-    case EPI_STORE: st4(a.C + row * a.ldc + n, v); break;
+    case EPI_STORE: st4(a.C + row * a.ldc + n, v); return v;
     case EPI_GATHER2: {
       const float* g = a.Wg + (int64_t)n * a.ldwg;
       v.x += g[zi] + g[a.S + zj]; g += a.ldwg;
@@ -66,26 +68,35 @@ __device__ __forceinline__ void gemm_epi4(const GemmArgs& a, int64_t row, int n,
       v.z += g[zi] + g[a.S + zj]; g += a.ldwg;
       v.w += g[zi] + g[a.S + zj];
       st4(a.C + row * a.ldc + n, v);
-    } break;
-    case EPI_Y_X:
+      return v;
+    }
+    case EPI_Y_X: {
       st4(a.C + row * a.ldc + n, v);
-      st4(a.C2 + row * a.ldc2 + n, make_float4(u * v.x, u * v.y, u * v.z, u * v.w));
-      break;
+      const float4 x = make_float4(u * v.x, u * v.y, u * v.z, u * v.w);
+      st4(a.C2 + row * a.ldc2 + n, x);
+      return x;
+    }
     case EPI_RESIDUAL: {
       st4(a.C + row * a.ldc + n, v);
       const float4 x = ld4(a.aux + row * a.ldaux + n);
       const float cu = a.c_new * u;
-      st4(a.C2 + row * a.ldc2 + n, make_float4(a.c_old * x.x + cu * v.x, a.c_old * x.y + cu * v.y, a.c_old * x.z + cu * v.z,
-                                               a.c_old * x.w + cu * v.w));
-    } break;
+      const float4 r = make_float4(a.c_old * x.x + cu * v.x, a.c_old * x.y + cu * v.y, a.c_old * x.z + cu * v.z,
+                                   a.c_old * x.w + cu * v.w);
+      st4(a.C2 + row * a.ldc2 + n, r);
+      return r;
+    }
     case EPI_DSILU: {
       const float4 z = ld4(a.aux + row * a.ldaux + n);
-      st4(a.C + row * a.ldc + n, make_float4(v.x * dsilu_f(z.x), v.y * dsilu_f(z.y), v.z * dsilu_f(z.z), v.w * dsilu_f(z.w)));
-    } break;
+      const float4 r = make_float4(v.x * dsilu_f(z.x), v.y * dsilu_f(z.y), v.z * dsilu_f(z.z), v.w * dsilu_f(z.w));
+      st4(a.C + row * a.ldc + n, r);
+      return r;
+    }
     case EPI_ACCUM: {
       const float4 c = ld4(a.C + row * a.ldc + n);
-      st4(a.C + row * a.ldc + n, make_float4(c.x + v.x, c.y + v.y, c.z + v.z, c.w + v.w));
-    } break;
+      const float4 r = make_float4(c.x + v.x, c.y + v.y, c.z + v.z, c.w + v.w);
+      st4(a.C + row * a.ldc + n, r);
+      return r;
+    }
     case EPI_SPLIT_RES:
       if (n < a.split) {
         const float4 x = ld4(a.aux + row * a.ldaux + n);
@@ -93,8 +104,9 @@ __device__ __forceinline__ void gemm_epi4(const GemmArgs& a, int64_t row, int n,
       } else {
         st4(a.C2 + row * a.ldc2 + (n - a.split), v);
       }
-      break;
+      return v;
   }
+  return v;
 }
 
 constexpr int GM = 128, GN = 64, GK = 16, GT = 256;
@@ -201,6 +213,11 @@ static __global__ void __launch_bounds__(GT) k_gemm(GemmArgs a) {
 }
 
 void launch_gemm_tc(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st);   // gemm_tc.cu
+// packed hi/lo B operand of a call site, built once and cached in the handle (gemm_tc.cu)
+float* packed_weights(Model* m, const GemmArgs& a, cudaStream_t st, int* Npad, int* Kpad);
+// a chain of up to 4 dependent GEMMs on the same 128-row tiles, activations kept in shared memory (gemm_chain.cu);
+// returns false when the shapes do not fit (caller launches the stages one by one)
+bool launch_gemm_chain(Model* m, const GemmArgs* stages, int n_stages, int64_t m_cap, cudaStream_t st);
 
 inline void launch_gemm(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st) {
   if (m_cap <= 0) return;

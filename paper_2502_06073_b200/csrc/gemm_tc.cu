@@ -22,6 +22,8 @@
 //     output row per thread, two warps per lane quadrant taking alternate 16-column groups) and applies the fused
 //     epilogue with 128-bit stores.
 #include <cstdint>
+#include <cstdio>
+#include <cstdlib>
 
 #include "gemm.cuh"
 
@@ -268,22 +270,27 @@ __global__ void __launch_bounds__(TC_T) k_gemm_tc(GemmArgs a, const float* __res
 
 }  // namespace
 
-void launch_gemm_tc(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st) {
+float* packed_weights(Model* m, const GemmArgs& a, cudaStream_t st, int* Npad_out, int* Kpad_out) {
   const int K = a.K0 + a.K1;
   const int Npad = (a.N + 15) / 16 * 16, Kpad = (K + TC_KC - 1) / TC_KC * TC_KC;
-  const int Nt = std::min(Npad, TC_NMAX);
-  // packed B operand, built once per call site
+  *Npad_out = Npad; *Kpad_out = Kpad;
   const std::array<int64_t, 5> key = {(int64_t)(a.W - m->d_w), a.ldw, a.wtrans, a.N, K};
-  float* Bp = nullptr;
   auto it = m->packed_w.find(key);
-  if (it == m->packed_w.end()) {
-    if (cudaMalloc(&Bp, sizeof(float) * 2 * (size_t)Npad * Kpad) != cudaSuccess) { cudaGetLastError(); m->err = "packed weight allocation failed"; return; }
-    const int64_t tot = (int64_t)Npad * Kpad;
-    k_pack_w<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(a.W, a.ldw, a.wtrans, a.N, K, Npad, Kpad, Bp);
-    m->packed_w[key] = Bp;
-  } else {
-    Bp = it->second;
-  }
+  if (it != m->packed_w.end()) return it->second;
+  float* Bp = nullptr;
+  if (cudaMalloc(&Bp, sizeof(float) * 2 * (size_t)Npad * Kpad) != cudaSuccess) { cudaGetLastError(); m->err = "packed weight allocation failed"; return nullptr; }
+  const int64_t tot = (int64_t)Npad * Kpad;
+  k_pack_w<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(a.W, a.ldw, a.wtrans, a.N, K, Npad, Kpad, Bp);
+  m->packed_w[key] = Bp;
+  return Bp;
+}
+
+void launch_gemm_tc(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st) {
+  const int K = a.K0 + a.K1;
+  int Npad, Kpad;
+  float* Bp = packed_weights(m, a, st, &Npad, &Kpad);
+  if (!Bp) return;
+  const int Nt = std::min(Npad, TC_NMAX);
   int tmem_cols = 32;
   while (tmem_cols < Nt) tmem_cols *= 2;
   const size_t smem = 2 * (size_t)(2 * TC_M * TC_KC * 4 + 2 * Nt * TC_KC * 4);
@@ -302,6 +309,361 @@ void launch_gemm_tc(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st)
   k_gemm_tc<<<grid, TC_T, smem, st>>>(a, Bp, Npad, Kpad, tmem_cols, vec_ok);
   prof_end(m, st);
   m->launches += 1;
+}
+
+}  // namespace allegro
+
+// =============================================================================================================
+// Chained GEMMs: up to CH_MAX dependent linears of one MLP on the same 128-row tile of edges.  The activation never
+// leaves the SM between stages: the epilogue of stage s reads the accumulator from TMEM, applies its fused epilogue
+// (global stores of what the backward pass needs), applies the prologue of stage s+1 and writes the result, split
+// hi/lo, straight into the canonical K-major UMMA layout of the next A operand.  The k loop therefore has no staging
+// work at all: one thread streams the pre-packed weight slices with cp.async.bulk (3 slots) and issues the MMAs.
+// =============================================================================================================
+namespace allegro {
+namespace {
+
+constexpr int CH_MAX = 4, CH_NB = 4, CH_KMAX = 128, CH_T = TC_T + 32;   // 8 compute warps + 1 weight-loader warp
+
+struct ChainArgs {
+  int n;
+  GemmArgs st[CH_MAX];
+  const float* Bp[CH_MAX];
+  const float* WgT[CH_MAX];      // EPI_GATHER2: species columns of W transposed, [2S][N]
+  int Npad[CH_MAX], Kpad[CH_MAX];
+};
+
+__device__ __forceinline__ float apply_pro(int pro, float v, float ascale) {
+  if (pro == PRO_SILU) return silu_f(v);
+  if (pro == PRO_SCALE_U) return v * ascale;
+  return v;
+}
+
+__global__ void k_transpose_wg(const float* __restrict__ Wg, int ldwg, int S, int N, float* __restrict__ out) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= 2 * (int64_t)S * N) return;
+  const int z = (int)(idx / N), n = (int)(idx - (int64_t)z * N);
+  out[idx] = Wg[(int64_t)n * ldwg + z];
+}
+
+__device__ __forceinline__ bool epi_needs_aux(const GemmArgs& a, int n) {
+  return a.epi == EPI_RESIDUAL || a.epi == EPI_DSILU || a.epi == EPI_ACCUM || (a.epi == EPI_SPLIT_RES && n < a.split);
+}
+// epilogue arithmetic of gemm_epi4 without the memory traffic: o1 -> C, o2 -> C2, pass -> next stage
+struct EpiOut { float4 o1, o2, pass; };
+__device__ __forceinline__ EpiOut chain_math(const GemmArgs& a, int n, float4 v, float u, float4 x, float4 gth) {
+  EpiOut r;
+  r.o1 = v; r.o2 = v; r.pass = v;
+  switch (a.epi) {
+    case EPI_GATHER2: v.x += gth.x; v.y += gth.y; v.z += gth.z; v.w += gth.w; r.o1 = v; r.pass = v; break;
+    case EPI_Y_X: r.o2 = make_float4(u * v.x, u * v.y, u * v.z, u * v.w); r.pass = r.o2; break;
+    case EPI_RESIDUAL: {
+      const float cu = a.c_new * u;
+      r.o2 = make_float4(a.c_old * x.x + cu * v.x, a.c_old * x.y + cu * v.y, a.c_old * x.z + cu * v.z, a.c_old * x.w + cu * v.w);
+      r.pass = r.o2;
+    } break;
+    case EPI_DSILU: r.o1 = make_float4(v.x * dsilu_f(x.x), v.y * dsilu_f(x.y), v.z * dsilu_f(x.z), v.w * dsilu_f(x.w)); r.pass = r.o1; break;
+    case EPI_ACCUM: r.o1 = make_float4(x.x + v.x, x.y + v.y, x.z + v.z, x.w + v.w); r.pass = r.o1; break;
+    case EPI_SPLIT_RES:
+      if (n < a.split) r.o1 = make_float4(a.c_old * x.x + v.x, a.c_old * x.y + v.y, a.c_old * x.z + v.z, a.c_old * x.w + v.w);
+      break;
+    default: break;
+  }
+  return r;
+}
+
+__device__ __forceinline__ void tmem_st4(uint32_t taddr, float4 x) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" ::"r"(taddr), "r"(__float_as_uint(x.x)),
+               "r"(__float_as_uint(x.y)), "r"(__float_as_uint(x.z)), "r"(__float_as_uint(x.w))
+               : "memory");
+}
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, float* v) {
+  uint32_t r[8];
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+               : "r"(taddr));
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+  for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
+}
+
+// A warp owns 32 rows; each thread computes 16 consecutive columns of its own row.  Global traffic goes through a
+// per-warp shared-memory tile [32][WT_LD] so that one instruction touches 8 rows x 64 contiguous bytes (full sectors)
+// instead of 32 rows x 16 bytes.
+constexpr int WT_LD = 20;
+__device__ __forceinline__ void warp_tile_store(float* tile, const float4 (&o)[4], int lane, float* C, int ld, int64_t rbase, int64_t M,
+                                                int col0, int N) {
+#pragma unroll
+  for (int j = 0; j < 4; ++j) *reinterpret_cast<float4*>(tile + lane * WT_LD + 4 * j) = o[j];
+  __syncwarp();
+  const int cq = (lane & 3) * 4;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int r = i * 8 + (lane >> 2);
+    const float4 t = *reinterpret_cast<const float4*>(tile + r * WT_LD + cq);
+    if (rbase + r < M && col0 + cq < N) *reinterpret_cast<float4*>(C + (rbase + r) * ld + col0 + cq) = t;
+  }
+  __syncwarp();
+}
+__device__ __forceinline__ void warp_tile_load(float* tile, float4 (&x)[4], int lane, const float* A, int ld, int64_t rbase, int64_t M,
+                                               int col0, int N) {
+  const int cq = (lane & 3) * 4;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int r = i * 8 + (lane >> 2);
+    float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (rbase + r < M && col0 + cq < N) t = *reinterpret_cast<const float4*>(A + (rbase + r) * ld + col0 + cq);
+    *reinterpret_cast<float4*>(tile + r * WT_LD + cq) = t;
+  }
+  __syncwarp();
+#pragma unroll
+  for (int j = 0; j < 4; ++j) x[j] = *reinterpret_cast<const float4*>(tile + lane * WT_LD + 4 * j);
+  __syncwarp();
+}
+
+// TMEM: columns [0, 128) accumulator D, columns [128, 256) the activation that feeds the current stage (fp32, prologue
+// already applied).  Shared memory: two 16-deep A staging buffers (hi | lo, canonical layout; reused as the per-warp
+// transposition tiles of the epilogue) and CH_NB weight slots filled by a dedicated loader warp.
+__global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ ChainArgs ca) {
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  __shared__ __align__(8) uint64_t mbar_mma[2];            // A staging buffer b free again
+  __shared__ __align__(8) uint64_t mbar_bfree[CH_NB];      // weight slot free again
+  __shared__ __align__(8) uint64_t mbar_b[CH_NB];          // weight slot landed
+  __shared__ uint32_t tmem_base_s;
+  const int64_t M = *ca.st[0].Mptr;
+  const int64_t row0 = (int64_t)blockIdx.x * TC_M;
+  if (row0 >= M) return;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  constexpr uint32_t a_floats = TC_M * TC_KC, slot_floats = 2 * TC_NMAX * TC_KC;
+  float* As = reinterpret_cast<float*>(smem_raw);          // [2][hi | lo]
+  float* Bs = As + 2 * 2 * a_floats;                        // [CH_NB][hi | lo]
+
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "r"(256));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  if (tid == 0) {
+    mbar_init(&mbar_mma[0], 1); mbar_init(&mbar_mma[1], 1);
+    for (int i = 0; i < CH_NB; ++i) { mbar_init(&mbar_b[i], 1); mbar_init(&mbar_bfree[i], 1); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  if (warp == 8) {
+    // weight loader: streams the pre-packed slices of every stage through the CH_NB slots, never blocking the issuer
+    if (lane == 0) {
+      int g = 0;
+      for (int s = 0; s < ca.n; ++s) {
+        const int Ntl = ca.Npad[s], nch = ca.Kpad[s] / TC_KC;
+        for (int c = 0; c < nch; ++c, ++g) {
+          const int slot = g % CH_NB, use = g / CH_NB;
+          if (use > 0) mbar_wait(&mbar_bfree[slot], (uint32_t)((use - 1) & 1));
+          bulk_g2s(Bs + slot * slot_floats, ca.Bp[s] + (int64_t)c * (2 * Ntl * TC_KC), (uint32_t)(2 * Ntl * TC_KC * 4), &mbar_b[slot]);
+        }
+      }
+    }
+    __syncthreads();   // matches the block-wide barrier before the TMEM release
+    return;
+  }
+  const uint32_t tmem_d = tmem_base_s, tmem_act = tmem_base_s + 128;
+  const int quad = warp & 3, half = warp >> 2;
+  const int erow = quad * 32 + lane;                       // this thread's row of the tile (TMEM lane)
+  const uint32_t lane_addr = (uint32_t)(quad * 32) << 16;
+  const int64_t row = row0 + erow, rbase = row0 + quad * 32;
+  const bool row_ok = row < M;
+  float* wtile = As + warp * (32 * WT_LD);                 // 640 floats per warp inside the 8192-float staging area
+  float u = 0.f; int zi = 0, zj = 0;
+  if (row_ok) {
+    const float* gq = ca.st[0].geo + row * GEO_W;
+    u = gq[4]; zi = __float_as_int(gq[6]); zj = __float_as_int(gq[7]);
+  }
+  // ---- stage-in: A of the first stage from global memory -> activation columns of TMEM (prologue applied)
+  {
+    const GemmArgs& a = ca.st[0];
+    const int ngrp = ca.Kpad[0] >> 4;
+    float ascale = 1.f;
+    if (a.pro == PRO_SCALE_U) ascale = a.c_new * u;
+#pragma unroll 1
+    for (int gk = half; gk < ngrp; gk += 2) {
+      const int k0 = gk * 16;
+      float4 x[4];
+      if (k0 < a.K0) warp_tile_load(wtile, x, lane, a.A0, a.lda0, rbase, M, k0, a.K0);
+      else warp_tile_load(wtile, x, lane, a.A1, a.lda1, rbase, M, k0 - a.K0, a.K1);
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+        tmem_st4(tmem_act + lane_addr + (uint32_t)(k0 + 4 * j),
+                 make_float4(apply_pro(a.pro, x[j].x, ascale), apply_pro(a.pro, x[j].y, ascale), apply_pro(a.pro, x[j].z, ascale),
+                             apply_pro(a.pro, x[j].w, ascale)));
+    }
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  asm volatile("bar.sync 1, 256;" ::: "memory");
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+
+  const int off_row = (erow >> 3) * (TC_KC / 4) * 32 + (erow & 7) * 4;
+  int gc = 0;                                               // global slice counter
+  for (int s = 0; s < ca.n; ++s) {
+    const GemmArgs& a = ca.st[s];
+    const int Nt = ca.Npad[s], nchunks = ca.Kpad[s] / TC_KC;
+    const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(Nt >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24);
+    const uint32_t b_bytes = (uint32_t)Nt * TC_KC * 4;
+#pragma unroll 1
+    for (int c = 0; c < nchunks; ++c) {
+      const int g = gc + c, b = g & 1;
+      if (g >= 2) mbar_wait(&mbar_mma[b], (uint32_t)(((g >> 1) - 1) & 1));   // MMAs of slice g-2 have drained buffer b
+      float* Ahi = As + b * 2 * a_floats;
+      float* Alo = Ahi + a_floats;
+      float v[8];
+      tmem_ld8(tmem_act + lane_addr + (uint32_t)(c * TC_KC + half * 8), v);
+#pragma unroll
+      for (int qq = 0; qq < 2; ++qq) {
+        float4 hi, lo;
+        hi.x = tf32_rna(v[4 * qq]); hi.y = tf32_rna(v[4 * qq + 1]); hi.z = tf32_rna(v[4 * qq + 2]); hi.w = tf32_rna(v[4 * qq + 3]);
+        lo.x = v[4 * qq] - hi.x; lo.y = v[4 * qq + 1] - hi.y; lo.z = v[4 * qq + 2] - hi.z; lo.w = v[4 * qq + 3] - hi.w;
+        *reinterpret_cast<float4*>(Ahi + off_row + (half * 2 + qq) * 32) = hi;
+        *reinterpret_cast<float4*>(Alo + off_row + (half * 2 + qq) * 32) = lo;
+      }
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      if (tid == 0) {
+        const int slot = g % CH_NB, use = g / CH_NB;
+        mbar_wait(&mbar_b[slot], (uint32_t)(use & 1));
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const uint32_t sa_hi = smem_u32(Ahi), sa_lo = smem_u32(Alo);
+        const uint32_t sb_hi = smem_u32(Bs + slot * slot_floats), sb_lo = sb_hi + b_bytes;
+        constexpr uint32_t sbo = (TC_KC / 4) * 128;
+#pragma unroll
+        for (int ks = 0; ks < TC_KC / 8; ++ks) {
+          const uint32_t koff = ks * 256;
+          const uint64_t dAh = umma_desc(sa_hi + koff, 128, sbo), dAl = umma_desc(sa_lo + koff, 128, sbo);
+          const uint64_t dBh = umma_desc(sb_hi + koff, 128, sbo), dBl = umma_desc(sb_lo + koff, 128, sbo);
+          umma_tf32(tmem_d, dAl, dBh, idesc, (c > 0 || ks > 0) ? 1u : 0u);
+          umma_tf32(tmem_d, dAh, dBl, idesc, 1u);
+          umma_tf32(tmem_d, dAh, dBh, idesc, 1u);
+        }
+        umma_commit(&mbar_mma[b]);
+        umma_commit(&mbar_bfree[slot]);
+      }
+    }
+    gc += nchunks;
+    {   // every slice issued: both staging buffers must have drained before they serve as transposition tiles
+      const int g = gc - 1;
+      mbar_wait(&mbar_mma[g & 1], (uint32_t)((g >> 1) & 1));
+      if (g >= 1) mbar_wait(&mbar_mma[(g - 1) & 1], (uint32_t)(((g - 1) >> 1) & 1));
+    }
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    // ---- epilogue of stage s; the value the next stage consumes goes back to TMEM with that stage's prologue applied
+    const bool last = (s + 1 == ca.n);
+    const int npro = last ? PRO_NONE : ca.st[s + 1].pro;
+    const float nscale = (!last && npro == PRO_SCALE_U) ? ca.st[s + 1].c_new * u : 1.f;
+    const bool two = (a.epi == EPI_Y_X || a.epi == EPI_RESIDUAL);
+#pragma unroll 1
+    for (int n0 = half * 16; n0 < Nt; n0 += 32) {
+      float4 x[4], o1[4], o2[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) x[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (epi_needs_aux(a, n0)) {
+        if (a.epi == EPI_ACCUM) warp_tile_load(wtile, x, lane, a.C, a.ldc, rbase, M, n0, a.N);
+        else warp_tile_load(wtile, x, lane, a.aux, a.ldaux, rbase, M, n0, a.N);
+      }
+      float v[16];
+      tmem_ld16(tmem_d + lane_addr + (uint32_t)n0, v);
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int n = n0 + j * 4;
+        float4 gth = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (a.epi == EPI_GATHER2 && n < a.N) {
+          const float4 g1 = *reinterpret_cast<const float4*>(ca.WgT[s] + (int64_t)zi * a.N + n);
+          const float4 g2 = *reinterpret_cast<const float4*>(ca.WgT[s] + (int64_t)(a.S + zj) * a.N + n);
+          gth = make_float4(g1.x + g2.x, g1.y + g2.y, g1.z + g2.z, g1.w + g2.w);
+        }
+        EpiOut r = chain_math(a, n, make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]), u, x[j], gth);
+        if (!row_ok || n >= a.N) r.pass = make_float4(0.f, 0.f, 0.f, 0.f);
+        o1[j] = r.o1; o2[j] = r.o2;
+        if (!last)
+          tmem_st4(tmem_act + lane_addr + (uint32_t)n, make_float4(apply_pro(npro, r.pass.x, nscale), apply_pro(npro, r.pass.y, nscale),
+                                                                  apply_pro(npro, r.pass.z, nscale), apply_pro(npro, r.pass.w, nscale)));
+      }
+      if (a.epi == EPI_SPLIT_RES && n0 >= a.split) {
+        warp_tile_store(wtile, o2, lane, a.C2, a.ldc2, rbase, M, n0 - a.split, a.N - a.split);
+      } else {
+        // the adjoint of a hidden layer is consumed by the next chained stage only: it never goes to global memory
+        if (!(a.epi == EPI_DSILU && !last)) warp_tile_store(wtile, o1, lane, a.C, a.ldc, rbase, M, n0, a.epi == EPI_SPLIT_RES ? a.split : a.N);
+        if (two) warp_tile_store(wtile, o2, lane, a.C2, a.ldc2, rbase, M, n0, a.N);
+      }
+    }
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    asm volatile("bar.sync 1, 256;" ::: "memory");
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  }
+  __syncthreads();
+  if (warp == 0) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_d), "r"(256));
+  }
+}
+
+}  // namespace
+}  // namespace allegro
+
+namespace allegro {
+
+bool launch_gemm_chain(Model* m, const GemmArgs* stages, int n_stages, int64_t m_cap, cudaStream_t st) {
+  if (!m->use_tc || !m->use_chain || n_stages < 1 || n_stages > CH_MAX || m_cap <= 0) return false;
+  ChainArgs ca{};
+  ca.n = n_stages;
+  auto al = [](const void* p) { return ((uintptr_t)p & 15) == 0; };
+  double work = 0;
+  int nmax = 16;
+  for (int s = 0; s < n_stages; ++s) {
+    const GemmArgs& a = stages[s];
+    const int K = a.K0 + a.K1;
+    if (K > CH_KMAX || a.N > TC_NMAX) return false;
+    if (s > 0 && (a.K1 != 0 || a.K0 != stages[s - 1].N)) return false;
+    bool vec_ok = (a.N % 4 == 0) && (a.ldc % 4 == 0) && al(a.C);
+    if (a.C2) vec_ok = vec_ok && (a.ldc2 % 4 == 0) && al(a.C2);
+    if (a.aux) vec_ok = vec_ok && (a.ldaux % 4 == 0) && al(a.aux);
+    if (a.epi == EPI_SPLIT_RES) vec_ok = vec_ok && (a.split % 16 == 0);
+    if (s == 0) {
+      vec_ok = vec_ok && (a.lda0 % 4 == 0) && al(a.A0) && (a.K0 % 4 == 0);
+      if (a.K1 > 0) vec_ok = vec_ok && (a.K0 % 16 == 0) && (a.lda1 % 4 == 0) && al(a.A1) && (a.K1 % 4 == 0);
+    }
+    if (!vec_ok) return false;
+  }
+  for (int s = 0; s < n_stages; ++s) {
+    ca.st[s] = stages[s];
+    ca.WgT[s] = nullptr;
+    if (stages[s].epi == EPI_GATHER2) {
+      // species columns of the first two-body matrix, transposed once: WgT[z][n] = Wg[n * ldwg + z], z < 2S
+      const GemmArgs& a = stages[s];
+      const std::array<int64_t, 5> key = {(int64_t)(a.Wg - m->d_w), a.ldwg, -7, a.N, a.S};
+      auto it = m->packed_w.find(key);
+      if (it == m->packed_w.end()) {
+        float* T = nullptr;
+        if (cudaMalloc(&T, sizeof(float) * 2 * (size_t)a.S * a.N) != cudaSuccess) { cudaGetLastError(); return false; }
+        const int64_t tot = 2 * (int64_t)a.S * a.N;
+        k_transpose_wg<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(a.Wg, a.ldwg, a.S, a.N, T);
+        it = m->packed_w.emplace(key, T).first;
+      }
+      ca.WgT[s] = it->second;
+    }
+    ca.Bp[s] = packed_weights(m, stages[s], st, &ca.Npad[s], &ca.Kpad[s]);
+    if (!ca.Bp[s]) return false;
+    nmax = std::max(nmax, ca.Npad[s]);
+    work += 2.0 * stages[s].N * (stages[s].K0 + stages[s].K1);
+  }
+  (void)nmax;
+  const size_t smem = (size_t)(2 * 2 * TC_M * TC_KC + CH_NB * 2 * TC_NMAX * TC_KC) * sizeof(float);   // 96 KB: two CTAs per SM
+  static bool attr_set = false;
+  if (!attr_set) { cudaFuncSetAttribute(k_gemm_chain, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_set = true; }
+  prof_begin(m, st, KC_GEMM, work);
+  k_gemm_chain<<<(unsigned)((m_cap + TC_M - 1) / TC_M), CH_T, smem, st>>>(ca);
+  prof_end(m, st);
+  m->launches += 1;
+  return true;
 }
 
 }  // namespace allegro

@@ -83,6 +83,7 @@ struct Model {
   int device = 0;
   int num_sms = 148;
   bool use_tc = true;              // dense linears on tcgen05 (3xTF32); ALLEGRO_GEMM=fp32 selects the FP32-pipe kernel
+  bool use_chain = true;           // MLP chains in one kernel (gemm_tc.cu k_gemm_chain); ALLEGRO_CHAIN=0 launches stage by stage
   bool use_tp3 = true;             // few-channel tensor-product kernels (tp3.cuh); ALLEGRO_TP=generic selects tp.cuh
   float* d_w = nullptr;            // weight blob
   float* d_weff = nullptr;         // collapsed edge-energy chain W_last...W_1 -> [D]

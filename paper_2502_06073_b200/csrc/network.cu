@@ -152,6 +152,19 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
   const unsigned gridE = (unsigned)((m_cap + T - 1) / T), gridWE = (unsigned)((m_cap * 32 + T - 1) / T);
   if (m_cap <= 0) return 0;
 
+  // Dependent linears are collected and launched as one chained kernel where the shapes allow (gemm_tc.cu)
+  std::vector<GemmArgs> ch;
+  auto flush = [&]() {
+    if (ch.empty()) return;
+    size_t i = 0;
+    while (i < ch.size()) {
+      const size_t cnt = std::min<size_t>(4, ch.size() - i);
+      if (!launch_gemm_chain(m, ch.data() + i, (int)cnt, m_cap, st))
+        for (size_t k = i; k < i + cnt; ++k) launch_gemm(m, ch[k], m_cap, st);
+      i += cnt;
+    }
+    ch.clear();
+  };
   // ---- F4: two-body MLP.  First layer = gather of the two one-hot columns + N_b-wide mat-vec.
   GemmArgs g;
   const int fan0 = 2 * S + Nb;
@@ -162,20 +175,21 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
     g.Wg = w + P.w_two_body[0]; g.ldwg = fan0; g.S = S; g.epi = EPI_GATHER2;
     if (hp.two_body_nl == 1) { m->err = "two_body MLP needs at least 2 linear layers"; return ALLEGRO_ERR_UNSUPPORTED; }
     g.C = ws.z2b[0]; g.ldc = hp.two_body_dims[0];
-    launch_gemm(m, g, m_cap, st);
+    ch.push_back(g);
     for (int i = 1; i < hp.two_body_nl; ++i) {
       g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo;
       g.A0 = ws.z2b[i - 1]; g.lda0 = g.K0 = hp.two_body_dims[i - 1]; g.pro = PRO_SILU;
       g.W = w + P.w_two_body[i]; g.ldw = hp.two_body_dims[i - 1]; g.N = hp.two_body_dims[i];
       if (i + 1 < hp.two_body_nl) { g.C = ws.z2b[i]; g.ldc = g.N; g.epi = EPI_STORE; }
       else { g.C = ws.y0; g.ldc = D; g.C2 = ws.x[0]; g.ldc2 = D; g.epi = EPI_Y_X; }   // x0 = u * y0
-      launch_gemm(m, g, m_cap, st);
+      ch.push_back(g);
     }
   }
   // ---- F5/F6 (layer 1): [W_init; W_env^1] x0 in one GEMM (adjacent in the blob)
   g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo;
   g.A0 = ws.x[0]; g.lda0 = g.K0 = D; g.W = w + P.w_init; g.ldw = D; g.N = 2 * nsc; g.C = ws.winit_w1; g.ldc = 2 * nsc;
-  launch_gemm(m, g, m_cap, st);
+  ch.push_back(g);
+  flush();
 
   std::vector<TpLayerDev> tps;
   std::vector<int> te_f(NL), te_b(NL), d3m(NL);
@@ -187,7 +201,8 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
     if (L >= 2) {   // F6
       g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo;
       g.A0 = ws.x[L - 1]; g.lda0 = g.K0 = D; g.W = w + ly.w_env; g.ldw = D; g.N = nsc; g.C = ws.wenv[L - 1]; g.ldc = nsc;
-      launch_gemm(m, g, m_cap, st);
+      ch.push_back(g);
+      flush();   // latent MLP of layer L-1 + this projection of its output
     }
     // F7
     prof_begin(m, st, KC_GAMMA, 0);
@@ -236,9 +251,10 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
         g.c_old = m->c_old[L - 1]; g.c_new = m->c_new[L - 1]; g.epi = EPI_RESIDUAL;
         if (hp.latent_nl == 1) { m->err = "latent MLP needs at least 2 linear layers"; return ALLEGRO_ERR_UNSUPPORTED; }
       }
-      launch_gemm(m, g, m_cap, st);
+      ch.push_back(g);
     }
   }
+  flush();
   // ---- F12
   prof_begin(m, st, KC_EDGE_MISC, 0);
   k_readout<<<gridWA, T, 0, st>>>(ws.rowptr_c, ws.x[NL], D, m->d_weff, species, a0, na, w + P.w_sigma, w + P.w_mu, m->e_atom.as<float>());
@@ -280,9 +296,10 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
           g.C = ws.xb[xcur ^ 1]; g.ldc = D; g.aux = ws.xb[xcur]; g.ldaux = D; g.c_old = c_old; g.split = D;
           g.C2 = ws.sb; g.ldc2 = nsc; g.epi = EPI_SPLIT_RES;
         }
-        launch_gemm(m, g, m_cap, st);
+        ch.push_back(g);
       }
     }
+    flush();
     xcur ^= 1;
     // B2 + B5: tensor-product backward -> Vbar^{L-1}, GE
     {
@@ -329,18 +346,15 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
     if (L >= 2) {   // B7: xbar^{L-1} += W_env^T wbar
       g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo; g.wtrans = 1;
       g.A0 = ws.wb; g.lda0 = g.K0 = nsc; g.W = w + ly.w_env; g.ldw = D; g.N = D; g.C = ws.xb[xcur]; g.ldc = D; g.epi = EPI_ACCUM;
-      launch_gemm(m, g, m_cap, st);
+      ch.push_back(g);
+      flush();
     }
   }
   // [W_init; W_env^1]^T [wbar_init; wbar^1] in one GEMM (B7 of layer 1 + B8; wbar_init comes from k_tp_bwd of layer 1)
   g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo; g.wtrans = 1;
   g.A0 = ws.wb; g.lda0 = g.K0 = 2 * nsc; g.W = w + P.w_init; g.ldw = D; g.N = D; g.C = ws.xb[xcur]; g.ldc = D; g.epi = EPI_ACCUM;
-  launch_gemm(m, g, m_cap, st);
-  // B9: ubar += xbar0 . y0;  two-body MLP backward with ybar0 = u xbar0
-  prof_begin(m, st, KC_EDGE_MISC, 0);
-  k_rowdot<<<gridWE, T, 0, st>>>(Mptr, ws.xb[xcur], ws.y0, D, 1.0f, 1, ws.ub);
-  prof_end(m, st);
-  m->launches += 1;
+  ch.push_back(g);
+  // two-body MLP backward with ybar0 = u xbar0, chained behind the accumulation above
   {
     const float* cur = ws.xb[xcur];
     int zc = 0;
@@ -351,14 +365,20 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
       if (i == hp.two_body_nl - 1) { g.pro = PRO_SCALE_U; g.c_new = 1.0f; }
       g.C = ws.zb[zc]; g.ldc = g.N; g.aux = ws.z2b[i - 1]; g.ldaux = g.N; g.epi = EPI_DSILU;
       cur = ws.zb[zc]; zc ^= 1;
-      launch_gemm(m, g, m_cap, st);
+      ch.push_back(g);
     }
     // bbar = W_1[:, 2S:]^T zbar_1
     g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo; g.wtrans = 1;
     g.A0 = cur; g.lda0 = g.K0 = hp.two_body_dims[0]; g.W = w + P.w_two_body[0] + 2 * S; g.ldw = fan0; g.N = Nb;
     g.C = ws.bb; g.ldc = Nb;
-    launch_gemm(m, g, m_cap, st);
+    ch.push_back(g);
   }
+  flush();
+  // B9: ubar += xbar0 . y0;  two-body MLP backward with ybar0 = u xbar0
+  prof_begin(m, st, KC_EDGE_MISC, 0);
+  k_rowdot<<<gridWE, T, 0, st>>>(Mptr, ws.xb[xcur], ws.y0, D, 1.0f, 1, ws.ub);
+  prof_end(m, st);
+  m->launches += 1;
   // B10, B11
   prof_begin(m, st, KC_EDGE_MISC, 0);
   k_edge_grad<<<gridE, T, 0, st>>>(Mptr, ws.geo, ws.bes, ws.bb, ws.ub, ws.yb, ws.e_lidx, Nb, hp.lmax, (float)hp.r_cut, m->g_list.as<float>());
