@@ -247,6 +247,42 @@ __global__ void k_xbar_init(const int64_t* __restrict__ Mptr, const float* __res
   xbar[idx] = sigma[__float_as_int(geo[e * GEO_W + 6])] * weff[d];
 }
 
+// B1 fused with the first B3 dot: xbar^{NL}[e, :] = sigma_{Z_i} w_eff and ubar[e] = c_new (xbar^{NL}_e . y^{NL}_e).  One warp per edge.
+__global__ void k_xbar_init_dot(const int64_t* __restrict__ Mptr, const float* __restrict__ geo, const float* __restrict__ sigma,
+                                const float* __restrict__ weff, int D, const float* __restrict__ y, float c_new,
+                                float* __restrict__ xbar, float* __restrict__ ubar) {
+  const int lane = threadIdx.x & 31;
+  const int64_t e = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (e >= *Mptr) return;
+  const float sg = sigma[__float_as_int(geo[e * GEO_W + 6])];
+  float s = 0.f;
+  for (int d = lane; d < D; d += 32) {
+    const float xb = sg * weff[d];
+    xbar[e * D + d] = xb;
+    s = fmaf(xb, y[e * D + d], s);
+  }
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+  if (lane == 0) ubar[e] = c_new * s;
+}
+
+// F12 with eps_e already formed by the GEMM epilogue: E_i = sigma_{Z_i} sum_row eps_e + mu_{Z_i}.  One warp per centre atom.
+__global__ void k_readout_eps(const int64_t* __restrict__ rowptr_c, const float* __restrict__ eps, const int* __restrict__ species,
+                              int64_t a0, int64_t n_atoms, const float* __restrict__ sigma, const float* __restrict__ mu,
+                              float* __restrict__ e_atom) {
+  const int lane = threadIdx.x & 31;
+  const int64_t a = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (a >= n_atoms) return;
+  float s = 0.f;
+  for (int64_t k = rowptr_c[a] + lane; k < rowptr_c[a + 1]; k += 32) s += eps[k];
+#pragma unroll
+  for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+  if (lane == 0) {
+    const int z = species[a0 + a];
+    e_atom[a0 + a] = sigma[z] * s + mu[z];
+  }
+}
+
 // out[e] (+)= scale * dot(A[e,:], B[e,:])   (ubar contributions of B3 and B9).  One warp per edge.
 __global__ void k_rowdot(const int64_t* __restrict__ Mptr, const float* __restrict__ A, const float* __restrict__ B, int D,
                          float scale, int accumulate, float* __restrict__ out) {

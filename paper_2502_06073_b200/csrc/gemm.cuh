@@ -29,6 +29,11 @@ struct GemmArgs {
   float c_old = 0.f, c_new = 1.f;   // PRO_SCALE_U multiplies by c_new * u;  EPI_RESIDUAL / EPI_SPLIT_RES use both
   const float* Wg = nullptr; int ldwg = 0, S = 0;      // EPI_GATHER2: += Wg[n*ldwg + zi] + Wg[n*ldwg + S + zj]
   int split = 0;                     // EPI_SPLIT_RES: columns < split -> C (residual), >= split -> C2
+  // optional row dot product fused into the chained epilogue (gemm_tc.cu; ignored by the single-GEMM kernels):
+  //   dot_out[e] = (dot_accum ? dot_out[e] : 0) + dot_scale * sum_n pass[e, n] * (dotv ? dotv[n] : dotB[e, n])
+  // where pass is the value the epilogue hands on (x^L for RESIDUAL, the accumulated sum for ACCUM, ...)
+  float* dot_out = nullptr; const float* dotv = nullptr; const float* dotB = nullptr; int lddot = 0;
+  float dot_scale = 1.f; int dot_accum = 0;
 };
 
 // one output element through the fused epilogue

@@ -430,6 +430,7 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
   __shared__ __align__(8) uint64_t mbar_bfree[CH_NB];      // weight slot free again
   __shared__ __align__(8) uint64_t mbar_b[CH_NB];          // weight slot landed
   __shared__ uint32_t tmem_base_s;
+  __shared__ float dot_s[TC_M];
   const int64_t M = *ca.st[0].Mptr;
   const int64_t row0 = (int64_t)blockIdx.x * TC_M;
   if (row0 >= M) return;
@@ -560,9 +561,11 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
     const int npro = last ? PRO_NONE : ca.st[s + 1].pro;
     const float nscale = (!last && npro == PRO_SCALE_U) ? ca.st[s + 1].c_new * u : 1.f;
     const bool two = (a.epi == EPI_Y_X || a.epi == EPI_RESIDUAL);
+    float dacc = 0.f;
 #pragma unroll 1
     for (int n0 = half * 16; n0 < Nt; n0 += 32) {
-      float4 x[4], o1[4], o2[4];
+      float4 x[4], o1[4], o2[4], yd[4];
+      if (a.dot_out && !a.dotv) warp_tile_load(wtile, yd, lane, a.dotB, a.lddot, rbase, M, n0, a.N);
 #pragma unroll
       for (int j = 0; j < 4; ++j) x[j] = make_float4(0.f, 0.f, 0.f, 0.f);
       if (epi_needs_aux(a, n0)) {
@@ -583,6 +586,10 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
         EpiOut r = chain_math(a, n, make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]), u, x[j], gth);
         if (!row_ok || n >= a.N) r.pass = make_float4(0.f, 0.f, 0.f, 0.f);
         o1[j] = r.o1; o2[j] = r.o2;
+        if (a.dot_out && n < a.N) {
+          const float4 y = a.dotv ? *reinterpret_cast<const float4*>(a.dotv + n) : yd[j];
+          dacc = fmaf(r.pass.x, y.x, fmaf(r.pass.y, y.y, fmaf(r.pass.z, y.z, fmaf(r.pass.w, y.w, dacc))));
+        }
         if (!last)
           tmem_st4(tmem_act + lane_addr + (uint32_t)n, make_float4(apply_pro(npro, r.pass.x, nscale), apply_pro(npro, r.pass.y, nscale),
                                                                   apply_pro(npro, r.pass.z, nscale), apply_pro(npro, r.pass.w, nscale)));
@@ -594,6 +601,11 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
         if (!(a.epi == EPI_DSILU && !last)) warp_tile_store(wtile, o1, lane, a.C, a.ldc, rbase, M, n0, a.epi == EPI_SPLIT_RES ? a.split : a.N);
         if (two) warp_tile_store(wtile, o2, lane, a.C2, a.ldc2, rbase, M, n0, a.N);
       }
+    }
+    if (a.dot_out) {   // the two warps that share a row quadrant combine their halves of the row dot product
+      if (half == 1) dot_s[erow] = dacc;
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      if (half == 0 && row_ok) a.dot_out[row] = (a.dot_accum ? a.dot_out[row] : 0.f) + a.dot_scale * (dacc + dot_s[erow]);
     }
     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -627,6 +639,8 @@ bool launch_gemm_chain(Model* m, const GemmArgs* stages, int n_stages, int64_t m
     if (a.C2) vec_ok = vec_ok && (a.ldc2 % 4 == 0) && al(a.C2);
     if (a.aux) vec_ok = vec_ok && (a.ldaux % 4 == 0) && al(a.aux);
     if (a.epi == EPI_SPLIT_RES) vec_ok = vec_ok && (a.split % 16 == 0);
+    if (a.dot_out && a.dotB) vec_ok = vec_ok && (a.lddot % 4 == 0) && al(a.dotB);
+    if (a.dot_out && a.dotv) vec_ok = vec_ok && al(a.dotv);
     if (s == 0) {
       vec_ok = vec_ok && (a.lda0 % 4 == 0) && al(a.A0) && (a.K0 % 4 == 0);
       if (a.K1 > 0) vec_ok = vec_ok && (a.K0 % 16 == 0) && (a.lda1 % 4 == 0) && al(a.A1) && (a.K1 % 4 == 0);

@@ -61,7 +61,7 @@ struct Workspace {       // per-chunk activations, sized for cap_edges active ed
   // backward
   float* xb[2] = {nullptr, nullptr}; float* zb[2] = {nullptr, nullptr};
   float* sb = nullptr; float* vb[2] = {nullptr, nullptr}; float* ge = nullptr; float* wb = nullptr;
-  float* yb = nullptr; float* ub = nullptr; float* bb = nullptr; float* gammab = nullptr;
+  float* yb = nullptr; float* ub = nullptr; float* eps = nullptr; float* bb = nullptr; float* gammab = nullptr;
 };
 
 // optional per-kernel-class timing with CUDA events on the launching stream (allegro_profile)

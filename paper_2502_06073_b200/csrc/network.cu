@@ -35,7 +35,7 @@ static void ws_sizes(const Plan& P, size_t* per_edge, size_t* per_atom) {
     maxv = std::max(maxv, std::max(ly.in_dim, ly.out_dim));
   }
   for (int i = 0; i + 1 < hp.two_body_nl; ++i) maxh = std::max(maxh, hp.two_body_dims[i]);
-  f += 2 * P.D + 2 * maxh + P.n_sc + 2 * (size_t)n * maxv + (size_t)n * P.d_sh + 2 * P.n_sc + P.d_sh + 1 + hp.n_bessel;
+  f += 2 * P.D + 2 * maxh + P.n_sc + 2 * (size_t)n * maxv + (size_t)n * P.d_sh + 2 * P.n_sc + P.d_sh + 2 + hp.n_bessel;
   *per_edge = f * sizeof(float) + 2 * sizeof(int) + sizeof(int64_t) + 64;
   *per_atom = ((size_t)NL + 1) * n * P.d_sh * sizeof(float) + sizeof(int) + sizeof(int64_t) + 64;
 }
@@ -91,6 +91,7 @@ int ws_prepare(Model* m, int64_t cap_edges, int64_t cap_atoms) {
   ws.wb = cf(E * 2 * P.n_sc);
   ws.yb = cf(E * P.d_sh);
   ws.ub = cf(E);
+  ws.eps = cf(E);
   ws.bb = cf(E * hp.n_bessel);
   ws.gammab = cf(A * n * P.d_sh);
   if (off > total) { m->err = "internal: workspace carve overflow"; return ALLEGRO_ERR_ALLOC; }
@@ -154,16 +155,19 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
 
   // Dependent linears are collected and launched as one chained kernel where the shapes allow (gemm_tc.cu)
   std::vector<GemmArgs> ch;
-  auto flush = [&]() {
-    if (ch.empty()) return;
+  auto flush = [&]() {   // returns true when every stage went through the chained kernel (fused row dots included)
+    bool all = true;
     size_t i = 0;
     while (i < ch.size()) {
       const size_t cnt = std::min<size_t>(4, ch.size() - i);
-      if (!launch_gemm_chain(m, ch.data() + i, (int)cnt, m_cap, st))
+      if (!launch_gemm_chain(m, ch.data() + i, (int)cnt, m_cap, st)) {
+        all = false;
         for (size_t k = i; k < i + cnt; ++k) launch_gemm(m, ch[k], m_cap, st);
+      }
       i += cnt;
     }
     ch.clear();
+    return all;
   };
   // ---- F4: two-body MLP.  First layer = gather of the two one-hot columns + N_b-wide mat-vec.
   GemmArgs g;
@@ -249,36 +253,41 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
       else {
         g.C = ws.ylat[L - 1]; g.ldc = D; g.C2 = ws.x[L]; g.ldc2 = D; g.aux = ws.x[L - 1]; g.ldaux = D;
         g.c_old = m->c_old[L - 1]; g.c_new = m->c_new[L - 1]; g.epi = EPI_RESIDUAL;
+        if (L == NL) { g.dot_out = ws.eps; g.dotv = m->d_weff; }   // F12: eps_e = w_eff . x^NL_e in the epilogue
         if (hp.latent_nl == 1) { m->err = "latent MLP needs at least 2 linear layers"; return ALLEGRO_ERR_UNSUPPORTED; }
       }
       ch.push_back(g);
     }
   }
-  flush();
+  const bool eps_fused = flush();
   // ---- F12
   prof_begin(m, st, KC_EDGE_MISC, 0);
-  k_readout<<<gridWA, T, 0, st>>>(ws.rowptr_c, ws.x[NL], D, m->d_weff, species, a0, na, w + P.w_sigma, w + P.w_mu, m->e_atom.as<float>());
+  if (eps_fused) k_readout_eps<<<gridWA, T, 0, st>>>(ws.rowptr_c, ws.eps, species, a0, na, w + P.w_sigma, w + P.w_mu, m->e_atom.as<float>());
+  else k_readout<<<gridWA, T, 0, st>>>(ws.rowptr_c, ws.x[NL], D, m->d_weff, species, a0, na, w + P.w_sigma, w + P.w_mu, m->e_atom.as<float>());
   prof_end(m, st);
   m->launches += 1;
 
   // ================= backward =================
   cudaMemsetAsync(ws.yb, 0, sizeof(float) * (size_t)m_cap * dsh, st);
   prof_begin(m, st, KC_EDGE_MISC, 0);
-  k_xbar_init<<<(unsigned)((m_cap * D + T - 1) / T), T, 0, st>>>(Mptr, ws.geo, w + P.w_sigma, m->d_weff, D, ws.xb[0]);   // B1
+  // B1 + the first B3 dot: xbar^NL = sigma w_eff;  ubar = c_new (xbar^NL . y^NL)
+  k_xbar_init_dot<<<gridWE, T, 0, st>>>(Mptr, ws.geo, w + P.w_sigma, m->d_weff, D, ws.ylat[NL - 1], m->c_new[NL - 1], ws.xb[0], ws.ub);
   m->launches += 1;
   prof_end(m, st);
   int xcur = 0, vcur = 0;
-  bool ub_init = false;
+  bool dot_done = true;   // the B3 dot of the layer about to be processed is already in ubar
   for (int L = NL; L >= 1; --L) {
     const Layer& ly = P.layers[L - 1];
     const TpLayerDev& tp = tps[L - 1];
     const float c_old = m->c_old[L - 1], c_new = m->c_new[L - 1];
     // B3: ubar += c_new (xbar . y)
-    prof_begin(m, st, KC_EDGE_MISC, 0);
-    k_rowdot<<<gridWE, T, 0, st>>>(Mptr, ws.xb[xcur], ws.ylat[L - 1], D, c_new, ub_init ? 1 : 0, ws.ub);
-    prof_end(m, st);
-    ub_init = true;
-    m->launches += 1;
+    if (!dot_done) {
+      prof_begin(m, st, KC_EDGE_MISC, 0);
+      k_rowdot<<<gridWE, T, 0, st>>>(Mptr, ws.xb[xcur], ws.ylat[L - 1], D, c_new, 1, ws.ub);
+      prof_end(m, st);
+      m->launches += 1;
+    }
+    dot_done = false;
     // B3/B4: latent MLP backward.  ybar = c_new u xbar is applied as the prologue of the first transposed GEMM.
     {
       const float* cur = ws.xb[xcur];
@@ -346,13 +355,16 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
     if (L >= 2) {   // B7: xbar^{L-1} += W_env^T wbar
       g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo; g.wtrans = 1;
       g.A0 = ws.wb; g.lda0 = g.K0 = nsc; g.W = w + ly.w_env; g.ldw = D; g.N = D; g.C = ws.xb[xcur]; g.ldc = D; g.epi = EPI_ACCUM;
+      // xbar^{L-1} is final here: the B3 dot of layer L-1 rides on this epilogue
+      g.dot_out = ws.ub; g.dotB = ws.ylat[L - 2]; g.lddot = D; g.dot_scale = m->c_new[L - 2]; g.dot_accum = 1;
       ch.push_back(g);
-      flush();
+      dot_done = flush();
     }
   }
   // [W_init; W_env^1]^T [wbar_init; wbar^1] in one GEMM (B7 of layer 1 + B8; wbar_init comes from k_tp_bwd of layer 1)
   g = GemmArgs(); g.Mptr = Mptr; g.geo = ws.geo; g.wtrans = 1;
   g.A0 = ws.wb; g.lda0 = g.K0 = 2 * nsc; g.W = w + P.w_init; g.ldw = D; g.N = D; g.C = ws.xb[xcur]; g.ldc = D; g.epi = EPI_ACCUM;
+  g.dot_out = ws.ub; g.dotB = ws.y0; g.lddot = D; g.dot_scale = 1.0f; g.dot_accum = 1;   // B9: ubar += xbar0 . y0
   ch.push_back(g);
   // two-body MLP backward with ybar0 = u xbar0, chained behind the accumulation above
   {
@@ -373,12 +385,12 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
     g.C = ws.bb; g.ldc = Nb;
     ch.push_back(g);
   }
-  flush();
-  // B9: ubar += xbar0 . y0;  two-body MLP backward with ybar0 = u xbar0
-  prof_begin(m, st, KC_EDGE_MISC, 0);
-  k_rowdot<<<gridWE, T, 0, st>>>(Mptr, ws.xb[xcur], ws.y0, D, 1.0f, 1, ws.ub);
-  prof_end(m, st);
-  m->launches += 1;
+  if (!flush()) {
+    prof_begin(m, st, KC_EDGE_MISC, 0);
+    k_rowdot<<<gridWE, T, 0, st>>>(Mptr, ws.xb[xcur], ws.y0, D, 1.0f, 1, ws.ub);
+    prof_end(m, st);
+    m->launches += 1;
+  }
   // B10, B11
   prof_begin(m, st, KC_EDGE_MISC, 0);
   k_edge_grad<<<gridE, T, 0, st>>>(Mptr, ws.geo, ws.bes, ws.bb, ws.ub, ws.yb, ws.e_lidx, Nb, hp.lmax, (float)hp.r_cut, m->g_list.as<float>());
