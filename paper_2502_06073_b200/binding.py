@@ -141,7 +141,7 @@ class Allegro:
             raise AllegroError(rc, _last_error(self._h))
 
     def close(self):
-        if getattr(self, "_h", None):
+        if getattr(self, "_h", None) and _lib is not None:   # _lib is None during interpreter shutdown
             _lib.allegro_destroy(self._h)
             self._h = None
 

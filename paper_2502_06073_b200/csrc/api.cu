@@ -230,7 +230,7 @@ int allegro_destroy(void* h) {
   for (CgDev& c : m->cg) { if (c.path_tab) cudaFree(c.path_tab); if (c.cg_idx) cudaFree(c.cg_idx); if (c.cg_val) cudaFree(c.cg_val); }
   NeighborList& nl = m->nl;
   for (DevBuf* b : {&nl.r_build, &nl.img, &nl.cell_of, &nl.cell_cnt, &nl.cell_start, &nl.cell_fill, &nl.sorted, &nl.row_cnt, &nl.rowptr,
-                    &nl.keys_tmp, &nl.keys, &nl.revpos, &nl.scan_tmp, &m->ws.arena, &m->ws.scan_tmp, &m->g_list, &m->e_atom, &m->e_partial,
+                    &nl.keys_tmp, &nl.keys, &nl.revpos, &nl.scan_tmp, &m->ws.arena, &m->ws.scan_tmp, &m->g_list, &m->e_atom, &m->e_partial, &m->act_total,
                     &m->flags, &m->md_pos, &m->md_vel, &m->md_mass, &m->md_species, &m->md_F, &m->md_E})
     free_buf(*b);
   delete m;
@@ -269,8 +269,7 @@ int allegro_energy_forces(void* h, const double* pos, const int32_t* species, in
   int rc = network_energy_forces(m, pos, species, N, E_out, F_out, E_atom_out, st);
   if (rc) return rc;
   int64_t act = 0;
-  if (N > 0 && m->ws.rowptr_c)
-    cudaMemcpyAsync(&act, m->ws.rowptr_c + std::min<int64_t>(N, m->ws.cap_atoms), sizeof(int64_t), cudaMemcpyDeviceToHost, st);
+  if (N > 0 && m->act_total.p) cudaMemcpyAsync(&act, m->act_total.p, sizeof(int64_t), cudaMemcpyDeviceToHost, st);
   rc = check_flags(m, st, "allegro_energy_forces");
   m->stats[0] = act; m->stats[2] = m->launches; m->stats[3] = 0; m->stats[4] = 1;
   return rc;
@@ -306,7 +305,7 @@ int allegro_md_step(void* h, double dt_fs, int64_t n_steps, void* stream) {
   if (rc) return rc;
   int64_t act = 0, elist = 0;
   if (m->nl.N > 0) {
-    cudaMemcpyAsync(&act, m->ws.rowptr_c + std::min<int64_t>(m->nl.N, m->ws.cap_atoms), sizeof(int64_t), cudaMemcpyDeviceToHost, st);
+    if (m->act_total.p) cudaMemcpyAsync(&act, m->act_total.p, sizeof(int64_t), cudaMemcpyDeviceToHost, st);
     cudaMemcpyAsync(&elist, m->nl.rowptr.as<int64_t>() + m->nl.N, sizeof(int64_t), cudaMemcpyDeviceToHost, st);
   }
   rc = check_flags(m, st, "allegro_md_step");

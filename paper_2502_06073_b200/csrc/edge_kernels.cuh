@@ -247,6 +247,9 @@ __global__ void k_xbar_init(const int64_t* __restrict__ Mptr, const float* __res
   xbar[idx] = sigma[__float_as_int(geo[e * GEO_W + 6])] * weff[d];
 }
 
+// active-edge counter of a force call, summed over its atom chunks
+__global__ void k_add_count(const int64_t* __restrict__ cnt, int64_t* __restrict__ total) { *total += *cnt; }
+
 // B1 fused with the first B3 dot: xbar^{NL}[e, :] = sigma_{Z_i} w_eff and ubar[e] = c_new (xbar^{NL}_e . y^{NL}_e).  One warp per edge.
 __global__ void k_xbar_init_dot(const int64_t* __restrict__ Mptr, const float* __restrict__ geo, const float* __restrict__ sigma,
                                 const float* __restrict__ weff, int D, const float* __restrict__ y, float c_new,

@@ -94,7 +94,7 @@ struct Model {
   NeighborList nl;
   Workspace ws;
   // global per-list-edge gradient and per-atom outputs
-  DevBuf g_list, e_atom, e_partial, flags, md_pos, md_vel, md_mass, md_species, md_F, md_E;
+  DevBuf g_list, e_atom, e_partial, act_total, flags, md_pos, md_vel, md_mass, md_species, md_F, md_E;
   bool md_ready = false;
   double md_cell[9] = {0};
   int64_t stats[8] = {0};

@@ -146,8 +146,9 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
   if (int rc = scan_counts(m, ws.act_cnt, ws.rowptr_c, na, &ws.scan_tmp, nullptr, st)) return rc;
   k_active<1><<<gridWA, T, 0, st>>>(pos, species, lv, a0, a1, hp.r_cut, hp.poly_p, Nb, nullptr, ws.rowptr_c, ws.e_center, ws.e_j,
                                     ws.e_lidx, ws.geo, ws.bes, m->g_list.as<float>(), ws.cap_edges, flags);
+  k_add_count<<<1, 1, 0, st>>>(ws.rowptr_c + na, m->act_total.as<int64_t>());
   prof_end(m, st);
-  m->launches += 2;
+  m->launches += 3;
   const int64_t* Mptr = ws.rowptr_c + na;
   const float* w = m->d_w;
   const unsigned gridE = (unsigned)((m_cap + T - 1) / T), gridWE = (unsigned)((m_cap * 32 + T - 1) / T);
@@ -405,6 +406,8 @@ int network_energy_forces(Model* m, const double* pos, const int32_t* species, i
   int* flags = m->flags.as<int>();
   if (int rc = ensure(m, &m->e_atom, sizeof(float) * (N + 1))) return rc;
   if (int rc = ensure(m, &m->e_partial, sizeof(double) * 1024)) return rc;
+  if (int rc = ensure(m, &m->act_total, sizeof(int64_t))) return rc;
+  cudaMemsetAsync(m->act_total.p, 0, sizeof(int64_t), st);
   const int T = 256;
   if (N > 0) {
     const double hs = 0.5 * nl.skin;
