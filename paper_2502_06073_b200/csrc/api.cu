@@ -131,7 +131,8 @@ int allegro_create(const float* weights_host, size_t n_weights, const allegro_hp
     delete m; return ALLEGRO_ERR_INVALID;
   }
   if (hp->n_channels % 4 != 0) { g_create_err = "n_channels must be a multiple of 4"; delete m; return ALLEGRO_ERR_UNSUPPORTED; }
-  if (hp->n_channels * P.d_sh > 1024) { g_create_err = "n_channels * (lmax+1)^2 must be <= 1024"; delete m; return ALLEGRO_ERR_UNSUPPORTED; }
+  if (hp->n_channels > 256) { g_create_err = "n_channels must be <= 256"; delete m; return ALLEGRO_ERR_UNSUPPORTED; }
+  if (hp->n_channels * P.d_sh > 4096) { g_create_err = "n_channels * (lmax+1)^2 must be <= 4096"; delete m; return ALLEGRO_ERR_UNSUPPORTED; }
   if (hp->two_body_nl < 2 || hp->latent_nl < 2) { g_create_err = "two-body and latent MLPs need >= 2 linear layers"; delete m; return ALLEGRO_ERR_UNSUPPORTED; }
   int ndev = 0;
   cudaError_t ce = cudaGetDeviceCount(&ndev);

@@ -102,45 +102,58 @@ __global__ void k_active(const double* __restrict__ pos, const int* __restrict__
   if (MODE == 0 && lane == 0) act_cnt[a - a0] = total;
 }
 
-// F7: Gamma_i[lm, c] = Nbar^-1/2 sum_{e in row(i)} w[e, l, c] Y_lm(rhat_e).  One block per centre atom; the
-// row's Y are staged in shared memory in slices of 32 edges; each thread owns outputs (lm, c), channel fastest
-// (w[e][l*n + c] and Gamma[a][lm][c] are read/written contiguously), and sums the row serially in CSR order
-// (deterministic, no atomics).
-__global__ void k_gamma(const int64_t* __restrict__ rowptr_c, const float* __restrict__ geo, const float* __restrict__ w, int ldw,
-                        int n, int lmax, float inv_sqrt_navg, float* __restrict__ gamma, int64_t n_atoms) {
+// F7: Gamma_i[lm, c] = Nbar^-1/2 sum_{e in row(i)} w[e, l, c] Y_lm(rhat_e).  One block per centre atom.  A thread owns a
+// channel c and every (256 / n)-th edge of the row: it forms w[e, l, c] Y_lm(e) for all lm in registers and sums over its
+// edges; the 256 / n partial sums per output are then added in a fixed order through shared memory (deterministic, no
+// atomics).  w[e][l*n + c] and Gamma[a][lm][c] are read / written contiguously in c.
+constexpr int GAMMA_T = 256;
+template <int LMAX>
+__global__ void __launch_bounds__(GAMMA_T) k_gamma_t(const int64_t* __restrict__ rowptr_c, const float* __restrict__ geo,
+                                                    const float* __restrict__ w, int ldw, int n, float inv_sqrt_navg,
+                                                    float* __restrict__ gamma, int64_t n_atoms) {
+  constexpr int DSH = (LMAX + 1) * (LMAX + 1);
+  __shared__ float red[GAMMA_T * (DSH + 1)];
   const int64_t a = blockIdx.x;
   if (a >= n_atoms) return;
-  __shared__ float Ys[32][16];
-  const int dsh = (lmax + 1) * (lmax + 1), nout = n * dsh;
   const int64_t b = rowptr_c[a], e = rowptr_c[a + 1];
-  constexpr int MAXO = 8;   // outputs per thread (n * d_sh <= 8 * blockDim)
-  float acc[MAXO];
+  const int epb = GAMMA_T / n;                  // edges in flight per pass (n <= 256)
+  const int c = threadIdx.x % n, grp = threadIdx.x / n;
+  float acc[DSH];
 #pragma unroll
-  for (int q = 0; q < MAXO; ++q) acc[q] = 0.f;
-  for (int64_t k0 = b; k0 < e; k0 += 32) {
-    const int cnt = (int)min((int64_t)32, e - k0);
-    __syncthreads();
-    if (threadIdx.x < cnt) {
-      const float* gq = geo + (k0 + threadIdx.x) * GEO_W;
-      sph_harm_rt(lmax, gq[0], gq[1], gq[2], Ys[threadIdx.x]);
-    }
-    __syncthreads();
+  for (int k = 0; k < DSH; ++k) acc[k] = 0.f;
+  if (grp < epb) {
+    for (int64_t k = b + grp; k < e; k += epb) {
+      const float* gq = geo + k * GEO_W;
+      float Y[16];
+      sph_harm<LMAX>(gq[0], gq[1], gq[2], Y);
+      const float* wk = w + k * ldw + c;
 #pragma unroll
-    for (int q = 0; q < MAXO; ++q) {
-      const int o = threadIdx.x + q * blockDim.x;
-      if (o < nout) {
-        const int lm = o / n, c = o - lm * n;
-        const int l = (lm >= 9) ? 3 : (lm >= 4) ? 2 : (lm >= 1) ? 1 : 0;
-        float s = 0.f;
-        for (int t = 0; t < cnt; ++t) s = fmaf(w[(k0 + t) * ldw + l * n + c], Ys[t][lm], s);
-        acc[q] += s;
+      for (int l = 0; l <= LMAX; ++l) {
+        const float wl = wk[l * n];
+#pragma unroll
+        for (int mm = 0; mm < 2 * l + 1; ++mm) acc[l * l + mm] = fmaf(wl, Y[l * l + mm], acc[l * l + mm]);
       }
     }
   }
 #pragma unroll
-  for (int q = 0; q < MAXO; ++q) {
-    const int o = threadIdx.x + q * blockDim.x;
-    if (o < nout) gamma[a * nout + o] = inv_sqrt_navg * acc[q];
+  for (int k = 0; k < DSH; ++k) red[threadIdx.x * (DSH + 1) + k] = acc[k];
+  __syncthreads();
+  const int nout = n * DSH;
+  for (int o = threadIdx.x; o < nout; o += GAMMA_T) {
+    const int lm = o / n, cc = o - lm * n;
+    float s = 0.f;
+    for (int g2 = 0; g2 < epb; ++g2) s += red[(g2 * n + cc) * (DSH + 1) + lm];
+    gamma[a * nout + o] = inv_sqrt_navg * s;
+  }
+}
+inline void launch_gamma(const int64_t* rowptr_c, const float* geo, const float* w, int ldw, int n, int lmax, float inv_sqrt_navg,
+                         float* gamma, int64_t n_atoms, cudaStream_t st) {
+  const unsigned g = (unsigned)n_atoms;
+  switch (lmax) {
+    case 0: k_gamma_t<0><<<g, GAMMA_T, 0, st>>>(rowptr_c, geo, w, ldw, n, inv_sqrt_navg, gamma, n_atoms); break;
+    case 1: k_gamma_t<1><<<g, GAMMA_T, 0, st>>>(rowptr_c, geo, w, ldw, n, inv_sqrt_navg, gamma, n_atoms); break;
+    case 2: k_gamma_t<2><<<g, GAMMA_T, 0, st>>>(rowptr_c, geo, w, ldw, n, inv_sqrt_navg, gamma, n_atoms); break;
+    default: k_gamma_t<3><<<g, GAMMA_T, 0, st>>>(rowptr_c, geo, w, ldw, n, inv_sqrt_navg, gamma, n_atoms); break;
   }
 }
 

@@ -211,7 +211,7 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
     }
     // F7
     prof_begin(m, st, KC_GAMMA, 0);
-    k_gamma<<<(unsigned)na, 128, 0, st>>>(ws.rowptr_c, ws.geo, ws.wenv[L - 1], ldw_env, n, hp.lmax, inv_sqrt_navg, ws.gamma[L - 1], na);
+    launch_gamma(ws.rowptr_c, ws.geo, ws.wenv[L - 1], ldw_env, n, hp.lmax, inv_sqrt_navg, ws.gamma[L - 1], na, st);
     prof_end(m, st);
     // F8, F9, F11
     int d3max = 1;
@@ -235,7 +235,7 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
       prof_begin(m, st, KC_TP_FWD, tp_work(P, L, false));
       if (tp3_supported(tp) && m->use_tp3) {
         const size_t sm3 = tp3_smem_bytes(tp, false);
-        const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(3, (200 * 1024) / std::max<size_t>(sm3, 1)));
+        const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(3, (227 * 1024) / (sm3 + 2048)));
         const int64_t nsub = (m_cap + 256 / n - 1) / (256 / n);
         launch_tp3(m->tp_sig[L - 1], false, (int)std::min<int64_t>(nsub, (int64_t)m->num_sms * per_sm), st, tp, io);
       } else {
@@ -334,7 +334,7 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
       prof_begin(m, st, KC_TP_BWD, tp_work(P, L, true));
       if (tp3_supported(tp) && m->use_tp3) {
         const size_t sm3 = tp3_smem_bytes(tp, true);
-        const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(2, (200 * 1024) / std::max<size_t>(sm3, 1)));
+        const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(3, (227 * 1024) / (sm3 + 2048)));
         const int64_t nsub = (m_cap + 256 / n - 1) / (256 / n);
         launch_tp3(m->tp_sig[L - 1], true, (int)std::min<int64_t>(nsub, (int64_t)m->num_sms * per_sm), st, tp, io);
       } else {

@@ -40,7 +40,7 @@ template <int N> struct RegAcc {
 // then per mixed irrep o: T_o[rows_o][K_o+4], rows_o = roundup(TE d3_o, 16), row = el d3 + m.
 // ---------------------------------------------------------------------------------------------------------
 template <int SIG>
-__global__ void __launch_bounds__(256) k_tp_fwd3(TpLayerDev ly, TpIo io) {
+__global__ void __launch_bounds__(256, 3) k_tp_fwd3(TpLayerDev ly, TpIo io) {
   using D = tpgen::SigDims<SIG>;
   extern __shared__ __align__(16) float sm[];
   __shared__ Tp3Smem g;
@@ -175,7 +175,7 @@ __global__ void __launch_bounds__(256) k_tp_fwd3(TpLayerDev ly, TpIo io) {
 // Layer 1 applies B8 in registers (wbar_init, Ybar) and never writes Vbar^0.
 // ---------------------------------------------------------------------------------------------------------
 template <int SIG>
-__global__ void __launch_bounds__(256) k_tp_bwd3(TpLayerDev ly, TpIo io) {
+__global__ void __launch_bounds__(256, 3) k_tp_bwd3(TpLayerDev ly, TpIo io) {
   using D = tpgen::SigDims<SIG>;
   extern __shared__ __align__(16) float sm[];
   __shared__ Tp3Smem g;
