@@ -323,6 +323,7 @@ void launch_gemm_tc(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st)
 namespace allegro {
 namespace {
 
+static_assert(true, "");
 constexpr int CH_MAX = 4, CH_NB = 4, CH_KMAX = 128, CH_T = TC_T + 32;   // 8 compute warps + 1 weight-loader warp
 
 struct ChainArgs {
@@ -426,8 +427,7 @@ __device__ __forceinline__ void warp_tile_load(float* tile, float4 (&x)[4], int 
 // transposition tiles of the epilogue) and CH_NB weight slots filled by a dedicated loader warp.
 __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ ChainArgs ca) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
-  __shared__ __align__(8) uint64_t mbar_mma[2];            // A staging buffer b free again
-  __shared__ __align__(8) uint64_t mbar_bfree[CH_NB];      // weight slot free again
+  __shared__ __align__(8) uint64_t mbar_s[CH_NB];          // slice g done (barrier g % CH_NB, phase g / CH_NB): frees A buffer and weight slot
   __shared__ __align__(8) uint64_t mbar_b[CH_NB];          // weight slot landed
   __shared__ uint32_t tmem_base_s;
   __shared__ float dot_s[TC_M];
@@ -444,8 +444,7 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
   if (tid == 0) {
-    mbar_init(&mbar_mma[0], 1); mbar_init(&mbar_mma[1], 1);
-    for (int i = 0; i < CH_NB; ++i) { mbar_init(&mbar_b[i], 1); mbar_init(&mbar_bfree[i], 1); }
+    for (int i = 0; i < CH_NB; ++i) { mbar_init(&mbar_b[i], 1); mbar_init(&mbar_s[i], 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -459,7 +458,7 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
         const int Ntl = ca.Npad[s], nch = ca.Kpad[s] / TC_KC;
         for (int c = 0; c < nch; ++c, ++g) {
           const int slot = g % CH_NB, use = g / CH_NB;
-          if (use > 0) mbar_wait(&mbar_bfree[slot], (uint32_t)((use - 1) & 1));
+          if (use > 0) mbar_wait(&mbar_s[slot], (uint32_t)((use - 1) & 1));   // slice g - CH_NB used this slot
           bulk_g2s(Bs + slot * slot_floats, ca.Bp[s] + (int64_t)c * (2 * Ntl * TC_KC), (uint32_t)(2 * Ntl * TC_KC * 4), &mbar_b[slot]);
         }
       }
@@ -513,7 +512,7 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
 #pragma unroll 1
     for (int c = 0; c < nchunks; ++c) {
       const int g = gc + c, b = g & 1;
-      if (g >= 2) mbar_wait(&mbar_mma[b], (uint32_t)(((g >> 1) - 1) & 1));   // MMAs of slice g-2 have drained buffer b
+      if (g >= 2) mbar_wait(&mbar_s[(g - 2) % CH_NB], (uint32_t)(((g - 2) / CH_NB) & 1));   // MMAs of slice g-2 have drained buffer b
       float* Ahi = As + b * 2 * a_floats;
       float* Alo = Ahi + a_floats;
       float v[8];
@@ -545,15 +544,14 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
           umma_tf32(tmem_d, dAh, dBl, idesc, 1u);
           umma_tf32(tmem_d, dAh, dBh, idesc, 1u);
         }
-        umma_commit(&mbar_mma[b]);
-        umma_commit(&mbar_bfree[slot]);
+        umma_commit(&mbar_s[slot]);
       }
     }
     gc += nchunks;
     {   // every slice issued: both staging buffers must have drained before they serve as transposition tiles
       const int g = gc - 1;
-      mbar_wait(&mbar_mma[g & 1], (uint32_t)((g >> 1) & 1));
-      if (g >= 1) mbar_wait(&mbar_mma[(g - 1) & 1], (uint32_t)(((g - 1) >> 1) & 1));
+      mbar_wait(&mbar_s[g % CH_NB], (uint32_t)((g / CH_NB) & 1));
+      if (g >= 1) mbar_wait(&mbar_s[(g - 1) % CH_NB], (uint32_t)(((g - 1) / CH_NB) & 1));
     }
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     // ---- epilogue of stage s; the value the next stage consumes goes back to TMEM with that stage's prologue applied
