@@ -32,6 +32,11 @@ struct GemmArgs {
   // optional row dot product fused into the chained epilogue (gemm_tc.cu; ignored by the single-GEMM kernels):
   //   dot_out[e] = (dot_accum ? dot_out[e] : 0) + dot_scale * sum_n pass[e, n] * (dotv ? dotv[n] : dotB[e, n])
   // where pass is the value the epilogue hands on (x^L for RESIDUAL, the accumulated sum for ACCUM, ...)
+  // rows of the GEMM may be (edge, m) pairs of one irrep of an equivariant tensor stored as [e][comp][c] (tp_big.cuh):
+  // M = *Mptr * m_mul rows; A0 row r / C row r live at tensor row (r / d3) * od + off + r % d3 when the map's d3 > 0
+  int m_mul = 1;
+  int amap_d3 = 0, amap_od = 0, amap_off = 0;
+  int cmap_d3 = 0, cmap_od = 0, cmap_off = 0;     // EPI_STORE only
   float* dot_out = nullptr; const float* dotv = nullptr; const float* dotB = nullptr; int lddot = 0;
   float dot_scale = 1.f; int dot_accum = 0;
 };
@@ -39,7 +44,10 @@ struct GemmArgs {
 // one output element through the fused epilogue
 __device__ __forceinline__ void gemm_epi(const GemmArgs& a, int64_t row, int n, float v, float u, int zi, int zj) {
   switch (a.epi) {
-    case EPI_STORE: a.C[row * a.ldc + n] = v; break;
+    case EPI_STORE: {
+      const int64_t r2 = a.cmap_d3 ? (row / a.cmap_d3) * a.cmap_od + a.cmap_off + row % a.cmap_d3 : row;
+      a.C[r2 * a.ldc + n] = v;
+    } break;
     case EPI_GATHER2:
       a.C[row * a.ldc + n] = v + a.Wg[(int64_t)n * a.ldwg + zi] + a.Wg[(int64_t)n * a.ldwg + a.S + zj];
       break;
@@ -65,7 +73,11 @@ __device__ __forceinline__ float4 gemm_epi4(const GemmArgs& a, int64_t row, int 
   auto ld4 = [](const float* p) { return *reinterpret_cast<const float4*>(p); };
   auto st4 = [](float* p, float4 x) { *reinterpret_cast<float4*>(p) = x; };
   switch (a.epi) {
-    case EPI_STORE: st4(a.C + row * a.ldc + n, v); return v;
+    case EPI_STORE: {
+      const int64_t r2 = a.cmap_d3 ? (row / a.cmap_d3) * a.cmap_od + a.cmap_off + row % a.cmap_d3 : row;
+      st4(a.C + r2 * a.ldc + n, v);
+      return v;
+    }
     case EPI_GATHER2: {
       const float* g = a.Wg + (int64_t)n * a.ldwg;
       v.x += g[zi] + g[a.S + zj]; g += a.ldwg;

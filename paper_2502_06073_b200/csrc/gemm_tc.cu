@@ -117,7 +117,7 @@ __global__ void __launch_bounds__(TC_T) k_gemm_tc(GemmArgs a, const float* __res
   __shared__ __align__(8) uint64_t mbar_mma[2];
   __shared__ __align__(8) uint64_t mbar_b[2];
   __shared__ uint32_t tmem_base_s;
-  const int64_t M = *a.Mptr;
+  const int64_t M = *a.Mptr * a.m_mul;
   const int64_t row0 = (int64_t)blockIdx.x * TC_M;
   if (row0 >= M) return;
   const int col0 = blockIdx.y * TC_NMAX;
@@ -147,8 +147,8 @@ __global__ void __launch_bounds__(TC_T) k_gemm_tc(GemmArgs a, const float* __res
   const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(Nt >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24);
 
   const int r = tid & 127, qh = tid >> 7;              // this thread stages row r, k-quads 2*qh and 2*qh+1 of each slice
-  const int64_t arow = row0 + r;
-  const bool arow_ok = arow < M;
+  const bool arow_ok = row0 + r < M;
+  const int64_t arow = a.amap_d3 ? ((row0 + r) / a.amap_d3) * a.amap_od + a.amap_off + (row0 + r) % a.amap_d3 : row0 + r;
   float ascale = 1.f;
   if (a.pro == PRO_SCALE_U && arow_ok) ascale = a.c_new * a.geo[arow * GEO_W + 4];
   const int off_row = (r >> 3) * (TC_KC / 4) * 32 + (r & 7) * 4;   // floats: (row/8)*SBO + (row%8)*16 B

@@ -61,7 +61,7 @@ struct Workspace {       // per-chunk activations, sized for cap_edges active ed
   // backward
   float* xb[2] = {nullptr, nullptr}; float* zb[2] = {nullptr, nullptr};
   float* sb = nullptr; float* vb[2] = {nullptr, nullptr}; float* ge = nullptr; float* wb = nullptr;
-  float* yb = nullptr; float* ub = nullptr; float* eps = nullptr; float* bb = nullptr; float* gammab = nullptr;
+  float* yb = nullptr; float* ub = nullptr; float* eps = nullptr; float* Tbig = nullptr; float* bb = nullptr; float* gammab = nullptr;
 };
 
 // optional per-kernel-class timing with CUDA events on the launching stream (allegro_profile)
@@ -84,6 +84,7 @@ struct Model {
   int num_sms = 148;
   bool use_tc = true;              // dense linears on tcgen05 (3xTF32); ALLEGRO_GEMM=fp32 selects the FP32-pipe kernel
   bool use_chain = true;           // MLP chains in one kernel (gemm_tc.cu k_gemm_chain); ALLEGRO_CHAIN=0 launches stage by stage
+  bool use_big = false;            // many-channel tensor product: T buffers + tcgen05 channel mixing (tp_big.cuh)
   bool use_tp3 = true;             // few-channel tensor-product kernels (tp3.cuh); ALLEGRO_TP=generic selects tp.cuh
   float* d_w = nullptr;            // weight blob
   float* d_weff = nullptr;         // collapsed edge-energy chain W_last...W_1 -> [D]

@@ -7,7 +7,7 @@
 #include "edge_kernels.cuh"
 #include "gemm.cuh"
 #include "model.h"
-#include "tp.cuh"
+#include "tp_big.cuh"
 
 namespace allegro {
 
@@ -16,7 +16,20 @@ size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 }
 
 // bytes of workspace per active edge / per atom of a chunk
-static void ws_sizes(const Plan& P, size_t* per_edge, size_t* per_atom) {
+// floats per edge of the per-irrep tensor-product buffers of the many-channel path (tp_big.cuh), max over layers
+static size_t tbig_per_edge(const Plan& P) {
+  size_t best = 0;
+  for (int L = 1; L < P.hp.n_layers; ++L) {
+    const Layer& ly = P.layers[L - 1];
+    size_t f = 0;
+    for (size_t o = 0; o < ly.out_irreps.size(); ++o)
+      if (ly.out_off[o] >= 0) f += (size_t)(2 * ly.out_irreps[o].l + 1) * ly.out_npaths[o] * P.hp.n_channels;
+    best = std::max(best, f);
+  }
+  return best;
+}
+
+static void ws_sizes(const Plan& P, bool big, size_t* per_edge, size_t* per_atom) {
   const allegro_hparams& hp = P.hp;
   const int n = hp.n_channels, NL = hp.n_layers;
   size_t f = GEO_W + hp.n_bessel;
@@ -36,6 +49,7 @@ static void ws_sizes(const Plan& P, size_t* per_edge, size_t* per_atom) {
   }
   for (int i = 0; i + 1 < hp.two_body_nl; ++i) maxh = std::max(maxh, hp.two_body_dims[i]);
   f += 2 * P.D + 2 * maxh + P.n_sc + 2 * (size_t)n * maxv + (size_t)n * P.d_sh + 2 * P.n_sc + P.d_sh + 2 + hp.n_bessel;
+  if (big) f += tbig_per_edge(P);
   *per_edge = f * sizeof(float) + 2 * sizeof(int) + sizeof(int64_t) + 64;
   *per_atom = ((size_t)NL + 1) * n * P.d_sh * sizeof(float) + sizeof(int) + sizeof(int64_t) + 64;
 }
@@ -49,7 +63,7 @@ int ws_prepare(Model* m, int64_t cap_edges, int64_t cap_atoms) {
   const allegro_hparams& hp = P.hp;
   const int n = hp.n_channels, NL = hp.n_layers;
   size_t pe, pa;
-  ws_sizes(P, &pe, &pa);
+  ws_sizes(P, m->use_big, &pe, &pa);
   const size_t total = pe * cap_edges + pa * (cap_atoms + 1) + (1 << 16);
   if (int rc = ensure(m, &ws.arena, total)) return rc;
   char* base = ws.arena.as<char>();
@@ -94,6 +108,7 @@ int ws_prepare(Model* m, int64_t cap_edges, int64_t cap_atoms) {
   ws.eps = cf(E);
   ws.bb = cf(E * hp.n_bessel);
   ws.gammab = cf(A * n * P.d_sh);
+  ws.Tbig = m->use_big ? cf(E * tbig_per_edge(P)) : nullptr;
   if (off > total) { m->err = "internal: workspace carve overflow"; return ALLEGRO_ERR_ALLOC; }
   ws.cap_edges = cap_edges; ws.cap_atoms = cap_atoms;
   return 0;
@@ -233,7 +248,24 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
     {
       dim3 grid((unsigned)((m_cap + TE - 1) / TE), (unsigned)(tp.has_lin ? tp.n_out : 1));
       prof_begin(m, st, KC_TP_FWD, tp_work(P, L, false));
-      if (tp3_supported(tp) && m->use_tp3) {
+      if (m->use_big && tpbig_supported(tp)) {
+        // many channels: tensor product to per-irrep T buffers, channel mixing as tcgen05 GEMMs written straight into V^L
+        TpBig big{};
+        size_t off = 0;
+        for (int o = 0; o < tp.n_out; ++o)
+          if (tp.has_lin && tp.out_off[o] >= 0) { big.T[o] = ws.Tbig + off; off += (size_t)ws.cap_edges * tp.out_d3[o] * tp.out_np[o] * n; }
+        launch_tpo(m->tp_sig[L - 1], false, m_cap, st, tp, io, big);
+        prof_end(m, st);
+        for (int o = 0; o < tp.n_out && tp.has_lin; ++o) {
+          if (tp.out_off[o] < 0) continue;
+          GemmArgs gm; gm.Mptr = Mptr; gm.geo = ws.geo; gm.m_mul = tp.out_d3[o];
+          gm.A0 = big.T[o]; gm.lda0 = gm.K0 = tp.out_np[o] * n;
+          gm.W = w + tp.wlin[o]; gm.ldw = tp.out_np[o] * n; gm.wtrans = 0; gm.N = n;
+          gm.C = ws.V[L - 1]; gm.ldc = n; gm.cmap_d3 = tp.out_d3[o]; gm.cmap_od = tp.out_dim; gm.cmap_off = tp.out_off[o];
+          launch_gemm(m, gm, m_cap * tp.out_d3[o], st);
+        }
+        prof_begin(m, st, KC_TP_FWD, 0);
+      } else if (tp3_supported(tp) && m->use_tp3) {
         const size_t sm3 = tp3_smem_bytes(tp, false);
         const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(3, (227 * 1024) / (sm3 + 2048)));
         const int64_t nsub = (m_cap + 256 / n - 1) / (256 / n);
@@ -332,7 +364,23 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
       io.wbar_init = ws.wb; io.ldwb = 2 * nsc; io.ybar = ws.yb;   // layer 1: B8 applied inside the kernel
       size_t smem = smem_of(TE, PC);
       prof_begin(m, st, KC_TP_BWD, tp_work(P, L, true));
-      if (tp3_supported(tp) && m->use_tp3) {
+      if (m->use_big && tpbig_supported(tp)) {
+        TpBig big{};
+        size_t off = 0;
+        for (int o = 0; o < tp.n_out; ++o)
+          if (tp.has_lin && tp.out_off[o] >= 0) { big.T[o] = ws.Tbig + off; off += (size_t)ws.cap_edges * tp.out_d3[o] * tp.out_np[o] * n; }
+        prof_end(m, st);
+        for (int o = 0; o < tp.n_out && tp.has_lin; ++o) {   // B2: Tbar_o = Vbar^L[., o, ., :] W_o
+          if (tp.out_off[o] < 0) continue;
+          GemmArgs gm; gm.Mptr = Mptr; gm.geo = ws.geo; gm.m_mul = tp.out_d3[o]; gm.wtrans = 1;
+          gm.A0 = io.vbar; gm.lda0 = n; gm.K0 = n; gm.amap_d3 = tp.out_d3[o]; gm.amap_od = tp.out_dim; gm.amap_off = tp.out_off[o];
+          gm.W = w + tp.wlin[o]; gm.ldw = tp.out_np[o] * n; gm.N = tp.out_np[o] * n;
+          gm.C = big.T[o]; gm.ldc = tp.out_np[o] * n;
+          launch_gemm(m, gm, m_cap * tp.out_d3[o], st);
+        }
+        prof_begin(m, st, KC_TP_BWD, 0);
+        launch_tpo(m->tp_sig[L - 1], true, m_cap, st, tp, io, big);
+      } else if (tp3_supported(tp) && m->use_tp3) {
         const size_t sm3 = tp3_smem_bytes(tp, true);
         const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(3, (227 * 1024) / (sm3 + 2048)));
         const int64_t nsub = (m_cap + 256 / n - 1) / (256 / n);
@@ -416,7 +464,7 @@ int network_energy_forces(Model* m, const double* pos, const int32_t* species, i
   }
   // single chunk when the workspace fits; otherwise atom chunks bounded by list edges (sized with the average row)
   size_t pe, pa;
-  ws_sizes(m->plan, &pe, &pa);
+  ws_sizes(m->plan, m->use_big, &pe, &pa);
   size_t free_b = 0, total_b = 0;
   cudaMemGetInfo(&free_b, &total_b);
   const size_t budget = (size_t)(0.80 * (double)(free_b + m->ws.arena.bytes));

@@ -86,6 +86,10 @@ void launch_tp_bwd(int sig, dim3 grid, size_t smem, cudaStream_t st, const TpLay
 size_t tp3_smem_bytes(const TpLayerDev& tp, bool backward);
 bool tp3_supported(const TpLayerDev& tp);
 void launch_tp3(int sig, bool backward, int grid, cudaStream_t st, const TpLayerDev& tp, const TpIo& io);
+struct TpBig;
+bool tpbig_supported(const TpLayerDev& tp);
+size_t tpbig_floats_per_edge(const TpLayerDev& tp);
+void launch_tpo(int sig, bool backward, int64_t m_cap, cudaStream_t st, const TpLayerDev& tp, const TpIo& io, const TpBig& big);
 
 constexpr int TP_MAXMT = 2;   // 4x4 micro-tiles per thread (forward): TE * d3 * n <= 8192
 constexpr int TP_MAXP = 16;   // paths into one output irrep

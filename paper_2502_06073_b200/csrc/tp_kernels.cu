@@ -1,6 +1,6 @@
 // tp_kernels.cu — instantiations of the generated tensor-product kernels (tp.cuh, tp3.cuh) and their launchers, in a
 // translation unit of their own: one instantiation per layer signature of tp_gen.cuh.
-#include "tp3.cuh"
+#include "tp_big.cuh"
 
 namespace allegro {
 
@@ -65,6 +65,31 @@ void launch_tp3(int sig, bool backward, int grid, cudaStream_t st, const TpLayer
       if (!attr_b[I]) { cudaFuncSetAttribute(k_tp_bwd3<I>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); attr_b[I] = true; } \
       k_tp_bwd3<I><<<grid, 256, smem, st>>>(tp, io);                                                                 \
     }                                                                                                                \
+    break;
+    TPGEN_FOR_EACH_SIG(X)
+#undef X
+    default: break;
+  }
+}
+
+// ---- many-channel path (tp_big.cuh)
+bool tpbig_supported(const TpLayerDev& tp) { return (tp.n == 64 || tp.n == 128 || tp.n == 256) && tp.n_out <= TP3_MAXO; }
+
+size_t tpbig_floats_per_edge(const TpLayerDev& tp) {
+  if (!tp.has_lin) return 0;
+  size_t f = 0;
+  for (int o = 0; o < tp.n_out; ++o)
+    if (tp.out_off[o] >= 0) f += (size_t)tp.out_d3[o] * tp.out_np[o] * tp.n;
+  return f;
+}
+
+void launch_tpo(int sig, bool backward, int64_t m_cap, cudaStream_t st, const TpLayerDev& tp, const TpIo& io, const TpBig& big) {
+  const unsigned grid = (unsigned)((m_cap * tp.n + 255) / 256);
+  switch (sig) {
+#define X(I)                                                                 \
+  case I:                                                                    \
+    if (!backward) k_tpo_fwd<I><<<grid, 256, 0, st>>>(tp, io, big);         \
+    else k_tpo_bwd<I><<<grid, 256, 0, st>>>(tp, io, big);                   \
     break;
     TPGEN_FOR_EACH_SIG(X)
 #undef X

@@ -118,7 +118,7 @@ def test_energy_forces_cfg0(lib):
     assert g.get_stats()["active_edges"] == 1880 or True
 
 
-@pytest.mark.parametrize("net", [(1, 1, 8), (2, 2, 8), (3, 3, 8), (3, 2, 4), (2, 3, 12), (3, 3, 16)])
+@pytest.mark.parametrize("net", [(1, 1, 8), (2, 2, 8), (3, 3, 8), (3, 2, 4), (2, 3, 12), (3, 3, 16), (2, 2, 64), (3, 3, 64)])
 @pytest.mark.parametrize("full_o3", [1, 0])
 def test_energy_forces_small_nets(lib, net, full_o3):
     """All (lmax, NL) plans incl. the unnatural-parity irreps of 3-layer full O(3); ragged widths; skin list."""
