@@ -187,7 +187,9 @@ def roofline_for(prof, stats, clocks, peaks, n_sm):
     except Exception:
         pass
     if dom in ("gemm", "tp_fwd", "tp_bwd"):
-        flops = prof[dom]["work"] * E_act                              # algorithmic flop of all launches of the class
+        # algorithmic flop of all launches of the class: `work` sums flop per edge over launches, and every launch
+        # covers one atom chunk, i.e. active_edges / chunks edges on average
+        flops = prof[dom]["work"] * E_act / max(1, stats.get("chunks", 1))
         ach = flops / (prof[dom]["ms"] * 1e-3) / 1e12
         common = {"achieved": ach, "unit": "TFLOP/s", "traffic": traffic, "launches": prof[dom]["launches"],
                   "avg_launch_ms": prof[dom]["ms"] / max(1, prof[dom]["launches"]),

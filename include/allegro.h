@@ -107,7 +107,8 @@ int allegro_get_neighbors(void* h, int64_t* rowptr, int32_t* col, int8_t* shift,
 
 /* Counters of the last energy_forces / md_step call (HOST int64 [8]): [0] active edges (r < r_cut) of
  * the last force evaluation, [1] list edges, [2] kernel launches of the call, [3] rebuilds of the call,
- * [4] force evaluations of the call, [5..7] reserved. */
+ * [4] force evaluations of the call, [5] atom chunks per force evaluation (the activation workspace is sized from the
+ * free device memory; chunks are exact because the model is strictly local), [6..7] reserved. */
 int allegro_get_stats(void* h, int64_t* stats);
 
 /* Per-kernel-class timing for bench.py's roofline line.  allegro_profile(h, 1) resets the counters and makes

@@ -194,7 +194,7 @@ class Allegro:
         s = np.zeros(8, np.int64)
         self._check(_lib.allegro_get_stats(self._h, s.ctypes.data))
         return dict(active_edges=int(s[0]), list_edges=int(s[1]), launches=int(s[2]), rebuilds=int(s[3]),
-                    force_evals=int(s[4]))
+                    force_evals=int(s[4]), chunks=max(1, int(s[5])))
 
     def profile(self, enable: bool):
         self._check(_lib.allegro_profile(self._h, 1 if enable else 0))

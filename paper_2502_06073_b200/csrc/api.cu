@@ -143,6 +143,7 @@ int allegro_create(const float* weights_host, size_t n_weights, const allegro_hp
   }
   cudaGetDevice(&m->device);
   { const char* g = std::getenv("ALLEGRO_GEMM"); m->use_tc = !(g && std::string(g) == "fp32"); }
+  { const char* g = std::getenv("ALLEGRO_GRAPH"); m->use_graph = !(g && std::string(g) == "0"); }
   { const char* g = std::getenv("ALLEGRO_CHAIN"); m->use_chain = !(g && std::string(g) == "0"); }
   { const char* g = std::getenv("ALLEGRO_TP"); m->use_tp3 = !(g && std::string(g) == "generic"); }
   m->use_big = m->use_tc && m->use_tp3 && (hp->n_channels == 64 || hp->n_channels == 128 || hp->n_channels == 256);
@@ -225,6 +226,8 @@ int allegro_create(const float* weights_host, size_t n_weights, const allegro_hp
 int allegro_destroy(void* h) {
   if (!h) return ALLEGRO_OK;
   Model* m = static_cast<Model*>(h);
+  md_graph_reset(m);
+  if (m->own_stream) cudaStreamDestroy(m->own_stream);
   if (m->d_w) cudaFree(m->d_w);
   if (m->d_weff) cudaFree(m->d_weff);
   for (cudaEvent_t e : m->prof.ev) cudaEventDestroy(e);

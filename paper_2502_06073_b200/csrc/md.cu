@@ -61,6 +61,8 @@ __global__ void k_kinetic_final(const double* __restrict__ partial, int nb, doub
 
 }  // namespace
 
+void md_graph_reset(Model* m);
+
 int md_init(Model* m, const double* pos, const double* vel, const double* mass, const int32_t* species, int64_t N,
             const double* cell, double cutoff, double skin, cudaStream_t st) {
   int rc = 0;
@@ -76,6 +78,7 @@ int md_init(Model* m, const double* pos, const double* vel, const double* mass, 
   cudaMemcpyAsync(m->md_mass.p, mass, sizeof(double) * N, cudaMemcpyDeviceToDevice, st);
   cudaMemcpyAsync(m->md_species.p, species, sizeof(int32_t) * N, cudaMemcpyDeviceToDevice, st);
   for (int k = 0; k < 9; ++k) m->md_cell[k] = cell[k];
+  md_graph_reset(m);   // buffers may move: the captured step is rebuilt on the next allegro_md_step
   if ((rc = nl_build(m, m->md_pos.as<double>(), N, cell, cutoff, skin, false, st))) return rc;
   m->nl.n_rebuilds = 0;
   if ((rc = network_energy_forces(m, m->md_pos.as<double>(), m->md_species.as<int32_t>(), N, m->md_E.as<double>(),
@@ -85,7 +88,8 @@ int md_init(Model* m, const double* pos, const double* vel, const double* mass, 
   return 0;
 }
 
-int md_step(Model* m, double dt, int64_t n_steps, cudaStream_t st) {
+// One velocity-Verlet step enqueued on st (no host synchronisation: the rebuild decision is a device flag).
+static int md_one_step(Model* m, double dt, cudaStream_t st) {
   NeighborList& nl = m->nl;
   const int64_t N = nl.N;
   int* flags = m->flags.as<int>();
@@ -95,22 +99,76 @@ int md_step(Model* m, double dt, int64_t n_steps, cudaStream_t st) {
   const int T = 256;
   const unsigned g3 = (unsigned)((3 * N + T - 1) / T), g1 = (unsigned)((N + T - 1) / T);
   const double hs = 0.5 * nl.skin;
-  for (int64_t s = 0; s < n_steps; ++s) {
-    prof_begin(m, st, KC_MD, 0);
-    k_kick_drift<<<g3, T, 0, st>>>(pos, vel, F, m->md_mass.as<double>(), N, dt, 1);
-    k_skin_test<<<g1, T, 0, st>>>(pos, nl.r_build.as<double>(), N, hs * hs, nl.skin == 0.0 ? 1 : 0, flags);
-    prof_end(m, st);
-    m->launches += 2;
-    prof_begin(m, st, KC_NEIGHBOR, 0);
-    if (int rc = nl_build(m, pos, N, m->md_cell, nl.cutoff, nl.skin, true, st)) return rc;
-    k_clear_flag<<<1, 1, 0, st>>>(flags, FLAG_REBUILD);
-    prof_end(m, st);
-    if (int rc = network_energy_forces(m, pos, m->md_species.as<int32_t>(), N, m->md_E.as<double>(), F, nullptr, st)) return rc;
-    prof_begin(m, st, KC_MD, 0);
-    k_kick_drift<<<g3, T, 0, st>>>(pos, vel, F, m->md_mass.as<double>(), N, dt, 0);
-    prof_end(m, st);
-    m->launches += 2;
+  prof_begin(m, st, KC_MD, 0);
+  k_kick_drift<<<g3, T, 0, st>>>(pos, vel, F, m->md_mass.as<double>(), N, dt, 1);
+  k_skin_test<<<g1, T, 0, st>>>(pos, nl.r_build.as<double>(), N, hs * hs, nl.skin == 0.0 ? 1 : 0, flags);
+  prof_end(m, st);
+  m->launches += 2;
+  prof_begin(m, st, KC_NEIGHBOR, 0);
+  if (int rc = nl_build(m, pos, N, m->md_cell, nl.cutoff, nl.skin, true, st)) return rc;
+  k_clear_flag<<<1, 1, 0, st>>>(flags, FLAG_REBUILD);
+  prof_end(m, st);
+  if (int rc = network_energy_forces(m, pos, m->md_species.as<int32_t>(), N, m->md_E.as<double>(), F, nullptr, st)) return rc;
+  prof_begin(m, st, KC_MD, 0);
+  k_kick_drift<<<g3, T, 0, st>>>(pos, vel, F, m->md_mass.as<double>(), N, dt, 0);
+  prof_end(m, st);
+  m->launches += 2;
+  return 0;
+}
+
+void md_graph_reset(Model* m) {
+  if (m->md_graph) { cudaGraphExecDestroy(m->md_graph); m->md_graph = nullptr; }
+  m->md_warm = false;
+}
+
+// n_steps steps.  The step is a fixed sequence of launches (conditional rebuild included), so after one plain step
+// (which performs every allocation and weight packing) it is captured once into a CUDA graph and replayed: the host
+// cost per step drops from ~50 launches to one cudaGraphLaunch.  Profiling runs (allegro_profile) and
+// ALLEGRO_GRAPH=0 use the plain path.  The legacy default stream cannot be captured: an internal blocking stream,
+// which the legacy stream orders itself with implicitly, carries the work instead.
+int md_step(Model* m, double dt, int64_t n_steps, cudaStream_t st) {
+  if (n_steps > 0 && m->use_graph && !m->prof.on && n_steps >= 2) {
+    if (st == nullptr) {
+      if (!m->own_stream && cudaStreamCreate(&m->own_stream) != cudaSuccess) { cudaGetLastError(); m->own_stream = nullptr; }
+      if (m->own_stream) st = m->own_stream;
+    }
+    if (st != nullptr) {
+      if (!m->md_warm) {
+        if (int rc = md_one_step(m, dt, st)) return rc;
+        m->md_warm = true;
+        --n_steps;
+      }
+      if (!m->md_graph || m->graph_dt != dt || m->graph_stream != st) {
+        if (m->md_graph) { cudaGraphExecDestroy(m->md_graph); m->md_graph = nullptr; }
+        const int64_t l0 = m->launches;
+        cudaGraph_t g = nullptr;
+        int rc = 0;
+        if (cudaStreamBeginCapture(st, cudaStreamCaptureModeRelaxed) == cudaSuccess) {
+          rc = md_one_step(m, dt, st);
+          cudaError_t ce = cudaStreamEndCapture(st, &g);
+          if (rc == 0 && ce == cudaSuccess && g && cudaGraphInstantiate(&m->md_graph, g, 0) == cudaSuccess) {
+            m->graph_dt = dt; m->graph_stream = st; m->graph_launches = m->launches - l0;
+          } else {
+            m->md_graph = nullptr;
+          }
+          if (g) cudaGraphDestroy(g);
+        }
+        cudaGetLastError();
+        m->launches = l0;
+        if (rc) return rc;
+      }
+      if (m->md_graph) {
+        for (int64_t s = 0; s < n_steps; ++s) {
+          if (cudaGraphLaunch(m->md_graph, st) != cudaSuccess) return cuda_fail(m, cudaGetLastError(), "cudaGraphLaunch");
+          m->launches += m->graph_launches;
+        }
+        m->stats[4] += n_steps;
+        return 0;
+      }
+    }
   }
+  for (int64_t s = 0; s < n_steps; ++s)
+    if (int rc = md_one_step(m, dt, st)) return rc;
   m->stats[4] += n_steps;
   return 0;
 }

@@ -97,6 +97,12 @@ struct Model {
   // global per-list-edge gradient and per-atom outputs
   DevBuf g_list, e_atom, e_partial, act_total, flags, md_pos, md_vel, md_mass, md_species, md_F, md_E;
   bool md_ready = false;
+  // CUDA-graph replay of one MD step (md.cu)
+  bool use_graph = true, md_warm = false;
+  cudaStream_t own_stream = nullptr, graph_stream = nullptr;
+  cudaGraphExec_t md_graph = nullptr;
+  double graph_dt = 0;
+  int64_t graph_launches = 0;
   double md_cell[9] = {0};
   int64_t stats[8] = {0};
   int64_t launches = 0;
@@ -132,5 +138,6 @@ int md_init(Model* m, const double* pos, const double* vel, const double* mass, 
             const double* cell, double cutoff, double skin, cudaStream_t st);
 int md_step(Model* m, double dt, int64_t n_steps, cudaStream_t st);
 int md_kinetic(Model* m, double* Ekin_dev, cudaStream_t st);
+void md_graph_reset(Model* m);
 
 }  // namespace allegro

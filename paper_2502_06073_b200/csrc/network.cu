@@ -492,6 +492,7 @@ int network_energy_forces(Model* m, const double* pos, const int32_t* species, i
   }
   if (E_atom_out && N > 0) cudaMemcpyAsync(E_atom_out, m->e_atom.p, sizeof(float) * N, cudaMemcpyDeviceToDevice, st);
   m->stats[1] = nl.E_list;
+  m->stats[5] = (N + atoms_per - 1) / std::max<int64_t>(atoms_per, 1);   // atom chunks of this force call
   return 0;
 }
 
