@@ -35,6 +35,77 @@ template <int N> struct RegAcc {
   __device__ __forceinline__ float operator()(int k) const { return r[k]; }
 };
 
+// One unit of the channel-mixing GEMM: 16 rows x (8 NB) output channels, K deep, 3-pass TF32 (hi/lo) with the A fragments
+// split on the fly and the pre-split B fragments read from shared memory (lo block at offset lo_off).  NB = n / 8.
+template <int NB>
+__device__ __forceinline__ void tp3_fwd_unit(const float* __restrict__ Ta, int ldk, const float* __restrict__ Bh, int lo_off, int ldn,
+                                             int K, int row_g, int d3, int TE, int64_t e0, int64_t M, float* __restrict__ out0,
+                                             int edge_stride, int n) {
+  float acc[NB][4];
+#pragma unroll
+  for (int nb = 0; nb < NB; ++nb)
+#pragma unroll
+    for (int j = 0; j < 4; ++j) acc[nb][j] = 0.f;
+  const float* ta = Ta;
+  const float* bh = Bh;
+  const int ldk8 = 8 * ldk, ldn4 = 4 * ldn, ldn8 = 8 * ldn;
+  for (int k0 = 0; k0 < K; k0 += 8) {
+    const float a[4] = {ta[0], ta[ldk8], ta[4], ta[ldk8 + 4]};
+    uint32_t ah[4], al[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { ah[j] = tf32_hi(a[j]); al[j] = __float_as_uint(a[j] - __uint_as_float(ah[j])); }
+#pragma unroll
+    for (int nb = 0; nb < NB; ++nb) {
+      const uint32_t b0h = __float_as_uint(bh[nb * 8]), b1h = __float_as_uint(bh[ldn4 + nb * 8]);
+      const uint32_t b0l = __float_as_uint(bh[lo_off + nb * 8]), b1l = __float_as_uint(bh[lo_off + ldn4 + nb * 8]);
+      mma_tf32(acc[nb], al, b0h, b1h);
+      mma_tf32(acc[nb], ah, b0l, b1l);
+      mma_tf32(acc[nb], ah, b0h, b1h);
+    }
+    ta += 8; bh += ldn8;
+  }
+  const DivS divd3(d3);
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    int e2, m;
+    divd3(row_g + 8 * h, &e2, &m);
+    if (e2 < TE && e0 + e2 < M) {
+      float* out = out0 + (e0 + e2) * edge_stride + m * n;
+#pragma unroll
+      for (int nb = 0; nb < NB; ++nb) *reinterpret_cast<float2*>(out + nb * 8) = make_float2(acc[nb][2 * h], acc[nb][2 * h + 1]);
+    }
+  }
+}
+
+// Backward unit: Tb[16 rows, K_o] = A[16 rows, n] B[n, K_o]; the A fragments of the KS = n / 8 k-steps are split once.
+template <int KS>
+__device__ __forceinline__ void tp3_bwd_unit(const float* __restrict__ A, int lda, const float* __restrict__ Bh, int lo_off, int ldb,
+                                             int K, float* __restrict__ Tb, int ldk) {
+  uint32_t ah[KS][4], al[KS][4];
+#pragma unroll
+  for (int ks = 0; ks < KS; ++ks) {
+    const float a[4] = {A[ks * 8], A[ks * 8 + 8 * lda], A[ks * 8 + 4], A[ks * 8 + 8 * lda + 4]};
+#pragma unroll
+    for (int j = 0; j < 4; ++j) { ah[ks][j] = tf32_hi(a[j]); al[ks][j] = __float_as_uint(a[j] - __uint_as_float(ah[ks][j])); }
+  }
+  const int ldb4 = 4 * ldb, ldb8 = 8 * ldb, ldk8 = 8 * ldk;
+  for (int nb8 = 0; nb8 < K; nb8 += 8) {
+    float acc[4] = {0.f, 0.f, 0.f, 0.f};
+    const float* bh = Bh + nb8;
+#pragma unroll
+    for (int ks = 0; ks < KS; ++ks) {
+      const uint32_t b0h = __float_as_uint(bh[0]), b1h = __float_as_uint(bh[ldb4]);
+      const uint32_t b0l = __float_as_uint(bh[lo_off]), b1l = __float_as_uint(bh[lo_off + ldb4]);
+      mma_tf32(acc, al[ks], b0h, b1h);
+      mma_tf32(acc, ah[ks], b0l, b1l);
+      mma_tf32(acc, ah[ks], b0h, b1h);
+      bh += ldb8;
+    }
+    *reinterpret_cast<float2*>(Tb + nb8) = make_float2(acc[0], acc[1]);
+    *reinterpret_cast<float2*>(Tb + ldk8 + nb8) = make_float2(acc[2], acc[3]);
+  }
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // forward.  smem (floats): per mixed irrep o: Bhi[K_o][n+8] | Blo[K_o][n+8]  (B[k][c'] = W_o[c'][k], k = pidx n + c),
 // then per mixed irrep o: T_o[rows_o][K_o+4], rows_o = roundup(TE d3_o, 16), row = el d3 + m.
@@ -83,6 +154,11 @@ __global__ void __launch_bounds__(256, 3) k_tp_fwd3(TpLayerDev ly, TpIo io) {
       Bh[k * ldn + cp] = hi; Bl[k * ldn + cp] = v - hi;
     }
   }
+  // this thread's slot in every T tile (irrep index is a compile-time constant in the unrolled path loop below)
+  float* tdst[D::NOUT];
+  int tld[D::NOUT];
+#pragma unroll
+  for (int o = 0; o < D::NOUT; ++o) { tld[o] = g.ldk[o]; tdst[o] = sm + g.toff[o] + (el * D::o_d3(o)) * g.ldk[o] + c; }
   for (int64_t st = blockIdx.x; st < nsub; st += gridDim.x) {
     const int64_t e0 = st * TE, e = e0 + el;
     __syncthreads();   // previous sub-tile's T fully consumed (and, first time, W_lin staged)
@@ -108,8 +184,9 @@ __global__ void __launch_bounds__(256, 3) k_tp_fwd3(TpLayerDev ly, TpIo io) {
         const int o = D::p_iro(p), pidx = D::p_pidx(p), d3 = D::o_d3(o);
         const bool lin = ly.has_lin && D::o_off(o) >= 0;
         if (!lin && o != 0) continue;
-        float* dst = sm + g.toff[o] + (el * d3) * g.ldk[o] + pidx * n + c;
-        const int ldk = g.ldk[o];
+        float* dst = tdst[o] + pidx * n;
+        const int ldk = tld[o];
+        (void)d3;
         float t0 = 0.f;
         tpgen::tp_path_fwd<SIG>(p, RegAcc<D::IN_DIM>{V}, RegAcc<D::DSH>{G}, [&](int m, float v) {
           if (lin) dst[m * ldk] = v;
@@ -126,44 +203,13 @@ __global__ void __launch_bounds__(256, 3) k_tp_fwd3(TpLayerDev ly, TpIo io) {
       int o = 0;
       while (u >= g.unit0[o + 1]) ++o;
       const int r0 = (u - g.unit0[o]) * 16, K = g.K[o], ldk = g.ldk[o], d3 = g.d3[o];
-      const float* T = sm + g.toff[o];
-      const float* Bh = sm + g.boff[o];
-      const float* Bl = Bh + K * ldn;
-      float acc[4][4];
-#pragma unroll
-      for (int nb = 0; nb < 4; ++nb)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) acc[nb][j] = 0.f;
-      const float* Ta = T + (r0 + gq) * ldk + tq;
-      for (int k0 = 0; k0 < K; k0 += 8) {
-        const float a[4] = {Ta[k0], Ta[k0 + 8 * ldk], Ta[k0 + 4], Ta[k0 + 8 * ldk + 4]};
-        uint32_t ah[4], al[4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) { ah[j] = tf32_hi(a[j]); al[j] = __float_as_uint(a[j] - __uint_as_float(ah[j])); }
-        const float* bh = Bh + (k0 + tq) * ldn + gq;
-        const float* bl = Bl + (k0 + tq) * ldn + gq;
-#pragma unroll
-        for (int nb = 0; nb < 4; ++nb) {
-          if (nb * 8 < n) {
-            const uint32_t b0h = __float_as_uint(bh[nb * 8]), b1h = __float_as_uint(bh[4 * ldn + nb * 8]);
-            const uint32_t b0l = __float_as_uint(bl[nb * 8]), b1l = __float_as_uint(bl[4 * ldn + nb * 8]);
-            mma_tf32(acc[nb], al, b0h, b1h);
-            mma_tf32(acc[nb], ah, b0l, b1l);
-            mma_tf32(acc[nb], ah, b0h, b1h);
-          }
-        }
-      }
-      const DivS divd3(d3);
-#pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        int e2, m;
-        divd3(r0 + gq + 8 * h, &e2, &m);
-        if (e2 < TE && e0 + e2 < M) {
-          float* out = io.vout + ((e0 + e2) * D::OUT_DIM + g.ooff[o] + m) * n + 2 * tq;
-#pragma unroll
-          for (int nb = 0; nb < 4; ++nb)
-            if (nb * 8 < n) *reinterpret_cast<float2*>(out + nb * 8) = make_float2(acc[nb][2 * h], acc[nb][2 * h + 1]);
-        }
+      const float* Ta = sm + g.toff[o] + (r0 + gq) * ldk + tq;
+      const float* Bh = sm + g.boff[o] + tq * ldn + gq;
+      float* out0 = io.vout + g.ooff[o] * n + 2 * tq;
+      switch (n >> 3) {
+        case 1: tp3_fwd_unit<1>(Ta, ldk, Bh, K * ldn, ldn, K, r0 + gq, d3, TE, e0, M, out0, D::OUT_DIM * n, n); break;
+        case 2: tp3_fwd_unit<2>(Ta, ldk, Bh, K * ldn, ldn, K, r0 + gq, d3, TE, e0, M, out0, D::OUT_DIM * n, n); break;
+        default: tp3_fwd_unit<4>(Ta, ldk, Bh, K * ldn, ldn, K, r0 + gq, d3, TE, e0, M, out0, D::OUT_DIM * n, n); break;
       }
     }
   }
@@ -221,6 +267,15 @@ __global__ void __launch_bounds__(256, 3) k_tp_bwd3(TpLayerDev ly, TpIo io) {
       Bh[cp * ldb + col] = hi; Bl[cp * ldb + col] = v - hi;
     }
   }
+  const float* tsrc[D::NOUT];
+  float* adst[D::NOUT];
+  int tld[D::NOUT];
+#pragma unroll
+  for (int o = 0; o < D::NOUT; ++o) {
+    tld[o] = g.ldk[o];
+    tsrc[o] = sm + g.toff[o] + (el * D::o_d3(o)) * g.ldk[o] + c;
+    adst[o] = sm + g.aoff[o] + (el * D::o_d3(o)) * lda + c;
+  }
   for (int64_t st = blockIdx.x; st < nsub; st += gridDim.x) {
     const int64_t e0 = st * TE, e = e0 + el;
     const bool valid = e < M;
@@ -230,7 +285,7 @@ __global__ void __launch_bounds__(256, 3) k_tp_bwd3(TpLayerDev ly, TpIo io) {
 #pragma unroll
       for (int o = 0; o < D::NOUT; ++o) {
         if (D::o_off(o) < 0) continue;
-        float* A = sm + g.aoff[o] + (el * D::o_d3(o)) * lda + c;
+        float* A = adst[o];
 #pragma unroll
         for (int m = 0; m < D::o_d3(o); ++m)
           A[m * lda] = valid ? io.vbar[(e * D::OUT_DIM + D::o_off(o) + m) * n + c] : 0.f;
@@ -243,34 +298,12 @@ __global__ void __launch_bounds__(256, 3) k_tp_bwd3(TpLayerDev ly, TpIo io) {
         while (u >= g.unit0[o + 1]) ++o;
         const int r0 = (u - g.unit0[o]) * 16, K = g.K[o], ldk = g.ldk[o], ldb = K + 8;
         const float* A = sm + g.aoff[o] + (r0 + gq) * lda + tq;
-        const float* Bh = sm + g.boff[o];
-        const float* Bl = Bh + n * ldb;
+        const float* Bh = sm + g.boff[o] + tq * ldb + gq;
         float* Tb = sm + g.toff[o] + (r0 + gq) * ldk + 2 * tq;
-        uint32_t ah[4][4], al[4][4];
-#pragma unroll
-        for (int ks = 0; ks < 4; ++ks) {
-          if (ks * 8 < n) {
-            const float a[4] = {A[ks * 8], A[ks * 8 + 8 * lda], A[ks * 8 + 4], A[ks * 8 + 8 * lda + 4]};
-#pragma unroll
-            for (int j = 0; j < 4; ++j) { ah[ks][j] = tf32_hi(a[j]); al[ks][j] = __float_as_uint(a[j] - __uint_as_float(ah[ks][j])); }
-          }
-        }
-        for (int nb = 0; nb * 8 < K; ++nb) {
-          float acc[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-          for (int ks = 0; ks < 4; ++ks) {
-            if (ks * 8 < n) {
-              const float* bh = Bh + (ks * 8 + tq) * ldb + nb * 8 + gq;
-              const float* bl = Bl + (ks * 8 + tq) * ldb + nb * 8 + gq;
-              const uint32_t b0h = __float_as_uint(bh[0]), b1h = __float_as_uint(bh[4 * ldb]);
-              const uint32_t b0l = __float_as_uint(bl[0]), b1l = __float_as_uint(bl[4 * ldb]);
-              mma_tf32(acc, al[ks], b0h, b1h);
-              mma_tf32(acc, ah[ks], b0l, b1l);
-              mma_tf32(acc, ah[ks], b0h, b1h);
-            }
-          }
-          *reinterpret_cast<float2*>(Tb + nb * 8) = make_float2(acc[0], acc[1]);
-          *reinterpret_cast<float2*>(Tb + 8 * ldk + nb * 8) = make_float2(acc[2], acc[3]);
+        switch (n >> 3) {
+          case 1: tp3_bwd_unit<1>(A, lda, Bh, n * ldb, ldb, K, Tb, ldk); break;
+          case 2: tp3_bwd_unit<2>(A, lda, Bh, n * ldb, ldb, K, Tb, ldk); break;
+          default: tp3_bwd_unit<4>(A, lda, Bh, n * ldb, ldb, K, Tb, ldk); break;
         }
       }
       __syncthreads();
@@ -308,8 +341,9 @@ __global__ void __launch_bounds__(256, 3) k_tp_bwd3(TpLayerDev ly, TpIo io) {
         const int o = D::p_iro(p), pidx = D::p_pidx(p), d3 = D::o_d3(o);
         const bool lin = ly.has_lin && D::o_off(o) >= 0;
         if (!lin && o != 0) continue;
-        const float* tb = sm + g.toff[o] + (el * d3) * g.ldk[o] + pidx * n + c;
-        const int ldk = g.ldk[o];
+        const float* tb = tsrc[o] + pidx * n;
+        const int ldk = tld[o];
+        (void)d3;
         const float sb = (o == 0) ? io.sbar[e * nsc + pidx * n + c] : 0.f;
         tpgen::tp_path_bwd<SIG>(p, RegAcc<D::IN_DIM>{V}, RegAcc<D::DSH>{G},
                                 [&](int m) { return (lin ? tb[m * ldk] : 0.f) + sb; },
