@@ -6,9 +6,11 @@
 
 namespace allegro {
 
-__device__ __forceinline__ float silu_f(float z) { return z / (1.0f + __expf(-z)); }
+// SiLU and its derivative with the fast reciprocal (MUFU.RCP, <= 2 ulp): the IEEE division costs ~10 more instructions
+// per element and the MLP epilogues are issue-bound (profiles/r1_c_launches.md)
+__device__ __forceinline__ float silu_f(float z) { return __fdividef(z, 1.0f + __expf(-z)); }
 __device__ __forceinline__ float dsilu_f(float z) {
-  float s = 1.0f / (1.0f + __expf(-z));
+  float s = __fdividef(1.0f, 1.0f + __expf(-z));
   return s * (1.0f + z * (1.0f - s));
 }
 

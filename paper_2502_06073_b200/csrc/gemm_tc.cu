@@ -324,7 +324,7 @@ namespace allegro {
 namespace {
 
 static_assert(true, "");
-constexpr int CH_MAX = 4, CH_NB = 4, CH_KMAX = 128, CH_T = TC_T + 32;   // 8 compute warps + 1 weight-loader warp
+constexpr int CH_MAX = 4, CH_NB = 4, CH_KMAX = 128, CH_T = TC_T + 64;   // 8 compute warps + weight-loader warp + MMA-issuer warp
 
 struct ChainArgs {
   int n;
@@ -429,6 +429,7 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t mbar_s[CH_NB];          // slice g done (barrier g % CH_NB, phase g / CH_NB): frees A buffer and weight slot
   __shared__ __align__(8) uint64_t mbar_b[CH_NB];          // weight slot landed
+  __shared__ __align__(8) uint64_t mbar_staged[2];         // A staging buffer b written by all 8 compute warps
   __shared__ uint32_t tmem_base_s;
   __shared__ float dot_s[TC_M];
   const int64_t M = *ca.st[0].Mptr;
@@ -445,6 +446,7 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
   }
   if (tid == 0) {
     for (int i = 0; i < CH_NB; ++i) { mbar_init(&mbar_b[i], 1); mbar_init(&mbar_s[i], 1); }
+    mbar_init(&mbar_staged[0], 8); mbar_init(&mbar_staged[1], 8);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -464,6 +466,40 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
       }
     }
     __syncthreads();   // matches the block-wide barrier before the TMEM release
+    return;
+  }
+  if (warp == 9) {
+    // MMA issuer: the only thread that talks to the tensor core.  It waits for a staged A slice (8 warp arrivals) and its
+    // weight slot, issues the 3 x 2 MMAs and commits them to the slice barrier; the compute warps never wait on it.
+    if (lane == 0) {
+      const uint32_t tmem_dd = tmem_base_s;
+      int g = 0;
+      for (int s = 0; s < ca.n; ++s) {
+        const int Nt = ca.Npad[s], nch = ca.Kpad[s] / TC_KC;
+        const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(Nt >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24);
+        const uint32_t b_bytes = (uint32_t)Nt * TC_KC * 4;
+        for (int c = 0; c < nch; ++c, ++g) {
+          const int b = g & 1, slot = g % CH_NB, use = g / CH_NB;
+          mbar_wait(&mbar_staged[b], (uint32_t)((g >> 1) & 1));
+          mbar_wait(&mbar_b[slot], (uint32_t)(use & 1));
+          asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+          const uint32_t sa_hi = smem_u32(As + b * 2 * a_floats), sa_lo = sa_hi + a_floats * 4;
+          const uint32_t sb_hi = smem_u32(Bs + slot * slot_floats), sb_lo = sb_hi + b_bytes;
+          constexpr uint32_t sbo = (TC_KC / 4) * 128;
+#pragma unroll
+          for (int ks = 0; ks < TC_KC / 8; ++ks) {
+            const uint32_t koff = ks * 256;
+            const uint64_t dAh = umma_desc(sa_hi + koff, 128, sbo), dAl = umma_desc(sa_lo + koff, 128, sbo);
+            const uint64_t dBh = umma_desc(sb_hi + koff, 128, sbo), dBl = umma_desc(sb_lo + koff, 128, sbo);
+            umma_tf32(tmem_dd, dAl, dBh, idesc, (c > 0 || ks > 0) ? 1u : 0u);
+            umma_tf32(tmem_dd, dAh, dBl, idesc, 1u);
+            umma_tf32(tmem_dd, dAh, dBh, idesc, 1u);
+          }
+          umma_commit(&mbar_s[slot]);
+        }
+      }
+    }
+    __syncthreads();
     return;
   }
   const uint32_t tmem_d = tmem_base_s, tmem_act = tmem_base_s + 128;
@@ -525,27 +561,10 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
         *reinterpret_cast<float4*>(Ahi + off_row + (half * 2 + qq) * 32) = hi;
         *reinterpret_cast<float4*>(Alo + off_row + (half * 2 + qq) * 32) = lo;
       }
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // this thread's stores -> visible to the tensor core
       asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-      asm volatile("bar.sync 1, 256;" ::: "memory");
-      if (tid == 0) {
-        const int slot = g % CH_NB, use = g / CH_NB;
-        mbar_wait(&mbar_b[slot], (uint32_t)(use & 1));
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        const uint32_t sa_hi = smem_u32(Ahi), sa_lo = smem_u32(Alo);
-        const uint32_t sb_hi = smem_u32(Bs + slot * slot_floats), sb_lo = sb_hi + b_bytes;
-        constexpr uint32_t sbo = (TC_KC / 4) * 128;
-#pragma unroll
-        for (int ks = 0; ks < TC_KC / 8; ++ks) {
-          const uint32_t koff = ks * 256;
-          const uint64_t dAh = umma_desc(sa_hi + koff, 128, sbo), dAl = umma_desc(sa_lo + koff, 128, sbo);
-          const uint64_t dBh = umma_desc(sb_hi + koff, 128, sbo), dBl = umma_desc(sb_lo + koff, 128, sbo);
-          umma_tf32(tmem_d, dAl, dBh, idesc, (c > 0 || ks > 0) ? 1u : 0u);
-          umma_tf32(tmem_d, dAh, dBl, idesc, 1u);
-          umma_tf32(tmem_d, dAh, dBh, idesc, 1u);
-        }
-        umma_commit(&mbar_s[slot]);
-      }
+      __syncwarp();
+      if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&mbar_staged[b])) : "memory");
     }
     gc += nchunks;
     {   // every slice issued: both staging buffers must have drained before they serve as transposition tiles
