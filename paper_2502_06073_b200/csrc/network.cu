@@ -313,14 +313,9 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
     const Layer& ly = P.layers[L - 1];
     const TpLayerDev& tp = tps[L - 1];
     const float c_old = m->c_old[L - 1], c_new = m->c_new[L - 1];
-    // B3: ubar += c_new (xbar . y)
-    if (!dot_done) {
-      prof_begin(m, st, KC_EDGE_MISC, 0);
-      k_rowdot<<<gridWE, T, 0, st>>>(Mptr, ws.xb[xcur], ws.ylat[L - 1], D, c_new, 1, ws.ub);
-      prof_end(m, st);
-      m->launches += 1;
-    }
-    dot_done = false;
+    // B3: ubar += c_new (xbar . y) rides on the epilogue that finalised xbar^L (xbar_init for L = NL, else the W_env^T
+    // accumulation still waiting in `ch`); the plain kernel below is the fallback when that stage could not be chained
+    const bool dot_pending = !dot_done;
     // B3/B4: latent MLP backward.  ybar = c_new u xbar is applied as the prologue of the first transposed GEMM.
     {
       const float* cur = ws.xb[xcur];
@@ -341,7 +336,15 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
         ch.push_back(g);
       }
     }
-    flush();
+    {
+      const bool chained = flush();
+      if (dot_pending && !chained) {
+        prof_begin(m, st, KC_EDGE_MISC, 0);
+        k_rowdot<<<gridWE, T, 0, st>>>(Mptr, ws.xb[xcur], ws.ylat[L - 1], D, c_new, 1, ws.ub);
+        prof_end(m, st);
+        m->launches += 1;
+      }
+    }
     xcur ^= 1;
     // B2 + B5: tensor-product backward -> Vbar^{L-1}, GE
     {
@@ -406,8 +409,8 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
       g.A0 = ws.wb; g.lda0 = g.K0 = nsc; g.W = w + ly.w_env; g.ldw = D; g.N = D; g.C = ws.xb[xcur]; g.ldc = D; g.epi = EPI_ACCUM;
       // xbar^{L-1} is final here: the B3 dot of layer L-1 rides on this epilogue
       g.dot_out = ws.ub; g.dotB = ws.ylat[L - 2]; g.lddot = D; g.dot_scale = m->c_new[L - 2]; g.dot_accum = 1;
-      ch.push_back(g);
-      dot_done = flush();
+      ch.push_back(g);   // not flushed: the latent-MLP backward of layer L-1 chains behind it
+      dot_done = false;
     }
   }
   // [W_init; W_env^1]^T [wbar_init; wbar^1] in one GEMM (B7 of layer 1 + B8; wbar_init comes from k_tp_bwd of layer 1)
