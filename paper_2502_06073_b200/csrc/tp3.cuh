@@ -110,12 +110,14 @@ __device__ __forceinline__ void tp3_bwd_unit(const float* __restrict__ A, int ld
 // forward.  smem (floats): per mixed irrep o: Bhi[K_o][n+8] | Blo[K_o][n+8]  (B[k][c'] = W_o[c'][k], k = pidx n + c),
 // then per mixed irrep o: T_o[rows_o][K_o+4], rows_o = roundup(TE d3_o, 16), row = el d3 + m.
 // ---------------------------------------------------------------------------------------------------------
-template <int SIG>
+// NCH = number of channels as a compile-time constant (8, 16, 32: strides become immediates, the kernels are issue-bound
+// and half of their instructions were address arithmetic), or 0 = read it from the layer descriptor.
+template <int SIG, int NCH>
 __global__ void __launch_bounds__(256, 3) k_tp_fwd3(TpLayerDev ly, TpIo io) {
   using D = tpgen::SigDims<SIG>;
   extern __shared__ __align__(16) float sm[];
   __shared__ Tp3Smem g;
-  const int n = ly.n, ldn = n + 8;
+  const int n = NCH ? NCH : ly.n, ldn = n + 8;
   const DivN divn(n);
   const int TE = 256 / n;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, gq = lane >> 2, tq = lane & 3;
@@ -220,12 +222,12 @@ __global__ void __launch_bounds__(256, 3) k_tp_fwd3(TpLayerDev ly, TpIo io) {
 // then per mixed irrep o: A_o[rows_o][n+4] (adjoint of V^L, row = el d3 + m) | Tb_o[rows_o][K_o+4] (adjoint of T).
 // Layer 1 applies B8 in registers (wbar_init, Ybar) and never writes Vbar^0.
 // ---------------------------------------------------------------------------------------------------------
-template <int SIG>
+template <int SIG, int NCH>
 __global__ void __launch_bounds__(256, 3) k_tp_bwd3(TpLayerDev ly, TpIo io) {
   using D = tpgen::SigDims<SIG>;
   extern __shared__ __align__(16) float sm[];
   __shared__ Tp3Smem g;
-  const int n = ly.n, lda = n + 4;
+  const int n = NCH ? NCH : ly.n, lda = n + 4;
   const DivN divn(n);
   const int TE = 256 / n;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, gq = lane >> 2, tq = lane & 3;

@@ -52,24 +52,13 @@ bool tp3_supported(const TpLayerDev& tp) {
   return tp3_smem_bytes(tp, true) <= 200 * 1024 && tp3_smem_bytes(tp, false) <= 200 * 1024;
 }
 
+void launch_tp3_fwd(int sig, int grid, size_t smem, cudaStream_t st, const TpLayerDev& tp, const TpIo& io);   // tp3_fwd.cu
+void launch_tp3_bwd(int sig, int grid, size_t smem, cudaStream_t st, const TpLayerDev& tp, const TpIo& io);   // tp3_bwd.cu
+
 void launch_tp3(int sig, bool backward, int grid, cudaStream_t st, const TpLayerDev& tp, const TpIo& io) {
-  static bool attr_f[tpgen::N_SIGS] = {false}, attr_b[tpgen::N_SIGS] = {false};
   const size_t smem = tp3_smem_bytes(tp, backward);
-  switch (sig) {
-#define X(I)                                                                                                         \
-  case I:                                                                                                            \
-    if (!backward) {                                                                                                 \
-      if (!attr_f[I]) { cudaFuncSetAttribute(k_tp_fwd3<I>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); attr_f[I] = true; } \
-      k_tp_fwd3<I><<<grid, 256, smem, st>>>(tp, io);                                                                 \
-    } else {                                                                                                         \
-      if (!attr_b[I]) { cudaFuncSetAttribute(k_tp_bwd3<I>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); attr_b[I] = true; } \
-      k_tp_bwd3<I><<<grid, 256, smem, st>>>(tp, io);                                                                 \
-    }                                                                                                                \
-    break;
-    TPGEN_FOR_EACH_SIG(X)
-#undef X
-    default: break;
-  }
+  if (backward) launch_tp3_bwd(sig, grid, smem, st, tp, io);
+  else launch_tp3_fwd(sig, grid, smem, st, tp, io);
 }
 
 // ---- many-channel path (tp_big.cuh)
