@@ -159,52 +159,87 @@ inline void launch_gamma(const int64_t* rowptr_c, const float* geo, const float*
 
 // B5 (row reduction) + B6: Gammabar_i = sum_row GE[e], then for every edge of the row
 //   wbar[e,l,c] = Nbar^-1/2 sum_m Gammabar[l,m,c] Y_lm(e);   Ybar[e,lm] += Nbar^-1/2 sum_c w[e,l,c] Gammabar[lm,c].
-// One block per centre atom, Gammabar kept in shared memory ([lm][n+1], padded against bank conflicts).
-__global__ void k_gammabar(const int64_t* __restrict__ rowptr_c, const float* __restrict__ geo, const float* __restrict__ ge,
-                           const float* __restrict__ w, int ldw, int n, int lmax, float inv_sqrt_navg,
-                           float* __restrict__ wbar, int ldwb, float* __restrict__ ybar, int64_t n_atoms) {
+// One block per centre atom, Gammabar kept in shared memory ([lm][n+1], padded against bank conflicts).  lmax and (for
+// n = 8, 16, 32) the channel count are compile-time constants: the kernel is issue-bound on address arithmetic otherwise.
+template <int LMAX, int NCH>
+__global__ void __launch_bounds__(128) k_gammabar_t(const int64_t* __restrict__ rowptr_c, const float* __restrict__ geo,
+                                                   const float* __restrict__ ge, const float* __restrict__ w, int ldw, int n_rt,
+                                                   float inv_sqrt_navg, float* __restrict__ wbar, int ldwb, float* __restrict__ ybar,
+                                                   int64_t n_atoms) {
   extern __shared__ float sm[];
+  constexpr int DSH = (LMAX + 1) * (LMAX + 1);
+  const int n = NCH ? NCH : n_rt;
   const int64_t a = blockIdx.x;
   if (a >= n_atoms) return;
-  const int dsh = (lmax + 1) * (lmax + 1), nout = n * dsh, ldg = n + 1;
-  float* Gb = sm;              // [dsh][n+1]
+  const int nout = n * DSH, ldg = n + 1;
+  float* Gb = sm;              // [DSH][n+1]
   const int64_t b = rowptr_c[a], e = rowptr_c[a + 1];
   const int len = (int)(e - b);
   if (len == 0) return;
-  for (int o = threadIdx.x; o < nout; o += blockDim.x) {
+  for (int o = threadIdx.x; o < nout; o += 128) {
     float s = 0.f;
-    for (int64_t k = b; k < e; ++k) s += ge[k * nout + o];
+    const float* gp = ge + b * nout + o;
+    for (int k = 0; k < len; ++k) s += gp[(int64_t)k * nout];
     const int lm = o / n, c = o - lm * n;
     Gb[lm * ldg + c] = s * inv_sqrt_navg;
   }
   __syncthreads();
   // wbar: one (edge, channel) pair per thread and iteration
-  for (int idx = threadIdx.x; idx < len * n; idx += blockDim.x) {
-    const int c = idx % n, kk = idx / n;
+  for (int idx = threadIdx.x; idx < len * n; idx += 128) {
+    const int kk = idx / n, c = idx - kk * n;
     const int64_t k = b + kk;
     const float* gq = geo + k * GEO_W;
     float Y[16];
-    sph_harm_rt(lmax, gq[0], gq[1], gq[2], Y);
+    sph_harm<LMAX>(gq[0], gq[1], gq[2], Y);
+    float* wo = wbar + k * ldwb + c;
 #pragma unroll
-    for (int l = 0; l < 4; ++l) {
-      if (l <= lmax) {
-        float s = 0.f;
+    for (int l = 0; l <= LMAX; ++l) {
+      float s = 0.f;
 #pragma unroll
-        for (int mm = 0; mm < 2 * l + 1; ++mm) s = fmaf(Gb[(l * l + mm) * ldg + c], Y[l * l + mm], s);
-        wbar[k * ldwb + l * n + c] = s;
-      }
+      for (int mm = 0; mm < 2 * l + 1; ++mm) s = fmaf(Gb[(l * l + mm) * ldg + c], Y[l * l + mm], s);
+      wo[l * n] = s;
     }
   }
   // Ybar: one (edge, lm) pair per thread and iteration
-  for (int idx = threadIdx.x; idx < len * dsh; idx += blockDim.x) {
-    const int lm = idx % dsh, kk = idx / dsh;
+  for (int idx = threadIdx.x; idx < len * DSH; idx += 128) {
+    const int kk = idx / DSH, lm = idx - kk * DSH;
     const int64_t k = b + kk;
     const int l = (lm >= 9) ? 3 : (lm >= 4) ? 2 : (lm >= 1) ? 1 : 0;
     const float* wk = w + k * ldw + l * n;
     const float* g = Gb + lm * ldg;
     float s = 0.f;
-    for (int c = 0; c < n; ++c) s = fmaf(wk[c], g[c], s);
-    ybar[k * dsh + lm] += s;
+    if (NCH) {
+#pragma unroll
+      for (int c = 0; c < (NCH ? NCH : 1); c += 4) {
+        const float4 w4 = *reinterpret_cast<const float4*>(wk + c);
+        s = fmaf(w4.x, g[c], fmaf(w4.y, g[c + 1], fmaf(w4.z, g[c + 2], fmaf(w4.w, g[c + 3], s))));
+      }
+    } else {
+      for (int c = 0; c < n; ++c) s = fmaf(wk[c], g[c], s);
+    }
+    ybar[k * DSH + lm] += s;
+  }
+}
+
+template <int LMAX>
+static void launch_gammabar_l(unsigned grid, size_t smem, cudaStream_t st, const int64_t* rowptr_c, const float* geo, const float* ge,
+                              const float* w, int ldw, int n, float inv, float* wbar, int ldwb, float* ybar, int64_t na) {
+  const bool vec = (ldw % 4 == 0) && ((((uintptr_t)w) & 15) == 0);
+  if (n == 8 && vec) k_gammabar_t<LMAX, 8><<<grid, 128, smem, st>>>(rowptr_c, geo, ge, w, ldw, n, inv, wbar, ldwb, ybar, na);
+  else if (n == 16 && vec) k_gammabar_t<LMAX, 16><<<grid, 128, smem, st>>>(rowptr_c, geo, ge, w, ldw, n, inv, wbar, ldwb, ybar, na);
+  else if (n == 32 && vec) k_gammabar_t<LMAX, 32><<<grid, 128, smem, st>>>(rowptr_c, geo, ge, w, ldw, n, inv, wbar, ldwb, ybar, na);
+  else k_gammabar_t<LMAX, 0><<<grid, 128, smem, st>>>(rowptr_c, geo, ge, w, ldw, n, inv, wbar, ldwb, ybar, na);
+}
+inline void launch_gammabar(const int64_t* rowptr_c, const float* geo, const float* ge, const float* w, int ldw, int n, int lmax,
+                            float inv, float* wbar, int ldwb, float* ybar, int64_t na, cudaStream_t st) {
+  const int dsh = (lmax + 1) * (lmax + 1);
+  const size_t smem = (size_t)(dsh * (n + 1) + 16) * sizeof(float);
+  const unsigned grid = (unsigned)na;
+  switch (lmax) {
+    case 0: launch_gammabar_l<0>(grid, smem, st, rowptr_c, geo, ge, w, ldw, n, inv, wbar, ldwb, ybar, na); break;
+    case 1: launch_gammabar_l<1>(grid, smem, st, rowptr_c, geo, ge, w, ldw, n, inv, wbar, ldwb, ybar, na); break;
+    case 2: launch_gammabar_l<2>(grid, smem, st, rowptr_c, geo, ge, w, ldw, n, inv, wbar, ldwb, ybar, na); break;
+    default: launch_gammabar_l<3>(grid, smem, st, rowptr_c, geo, ge, w, ldw, n, inv, wbar, ldwb, ybar, na); break;
   }
 }
 
@@ -280,6 +315,28 @@ __global__ void k_xbar_init_dot(const int64_t* __restrict__ Mptr, const float* _
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
   if (lane == 0) ubar[e] = c_new * s;
+}
+
+// Same, D a multiple of 4 with D / 4 a power of two <= 32: D / 4 threads per edge, 128-bit accesses.
+__global__ void k_xbar_init_dot4(const int64_t* __restrict__ Mptr, const float* __restrict__ geo, const float* __restrict__ sigma,
+                                 const float* __restrict__ weff, int D, const float* __restrict__ y, float c_new,
+                                 float* __restrict__ xbar, float* __restrict__ ubar) {
+  const int q4 = D >> 2;
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t e = idx / q4;
+  const int q = (int)(idx - e * q4);
+  const bool valid = e < *Mptr;
+  float s = 0.f;
+  if (valid) {
+    const float sg = sigma[__float_as_int(geo[e * GEO_W + 6])];
+    const float4 w4 = *reinterpret_cast<const float4*>(weff + 4 * q);
+    const float4 y4 = *reinterpret_cast<const float4*>(y + e * D + 4 * q);
+    const float4 xb = make_float4(sg * w4.x, sg * w4.y, sg * w4.z, sg * w4.w);
+    *reinterpret_cast<float4*>(xbar + e * D + 4 * q) = xb;
+    s = fmaf(xb.x, y4.x, fmaf(xb.y, y4.y, fmaf(xb.z, y4.z, xb.w * y4.w)));
+  }
+  for (int d = q4 >> 1; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+  if (q == 0 && valid) ubar[e] = c_new * s;
 }
 
 // F12 with eps_e already formed by the GEMM epilogue: E_i = sigma_{Z_i} sum_row eps_e + mu_{Z_i}.  One warp per centre atom.

@@ -55,12 +55,56 @@ __global__ void k_scan_add(int64_t* __restrict__ out, const int64_t* __restrict_
   else if (i == n && total) out[n] = *total;
 }
 
+// small inputs: one block walks the array in slices of SCAN_T with a running carry (one launch instead of five)
+__global__ void __launch_bounds__(SCAN_T) k_scan_small(const int* __restrict__ cnt, int64_t* __restrict__ out, int64_t n, const int* flag) {
+  if (flag && *flag == 0) return;
+  __shared__ int64_t warp_tot[32];
+  __shared__ int64_t carry_s;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (threadIdx.x == 0) carry_s = 0;
+  __syncthreads();
+  for (int64_t i0 = 0; i0 < n; i0 += SCAN_T) {
+    const int64_t i = i0 + threadIdx.x;
+    const int64_t v = (i < n) ? (int64_t)cnt[i] : 0;
+    int64_t x = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const int64_t y = __shfl_up_sync(0xffffffffu, x, d);
+      if (lane >= d) x += y;
+    }
+    if (lane == 31) warp_tot[wid] = x;
+    __syncthreads();
+    if (wid == 0) {
+      int64_t t = warp_tot[lane];
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const int64_t y = __shfl_up_sync(0xffffffffu, t, d);
+        if (lane >= d) t += y;
+      }
+      warp_tot[lane] = t;
+    }
+    __syncthreads();
+    const int64_t carry = carry_s;
+    const int64_t base = carry + (wid ? warp_tot[wid - 1] : 0);
+    if (i < n) out[i] = base + x - v;
+    __syncthreads();
+    if (threadIdx.x == SCAN_T - 1) carry_s = base + x;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) out[n] = carry_s;
+}
+
 }  // namespace
 
 // out[0..n] = exclusive scan of cnt[0..n-1] (out[n] = total).  Three levels of 1024 (n <= 2^30).
 int scan_counts(Model* m, const int* cnt, int64_t* out, int64_t n, DevBuf* tmp, const int* flag, cudaStream_t st) {
   if (n <= 0) {
     cudaMemsetAsync(out, 0, sizeof(int64_t), st);
+    return 0;
+  }
+  if (n <= 16 * SCAN_T) {
+    k_scan_small<<<1, SCAN_T, 0, st>>>(cnt, out, n, flag);
+    m->launches += 1;
     return 0;
   }
   const int64_t nb1 = (n + SCAN_T - 1) / SCAN_T, nb2 = (nb1 + SCAN_T - 1) / SCAN_T, nb3 = (nb2 + SCAN_T - 1) / SCAN_T;

@@ -304,7 +304,11 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
   cudaMemsetAsync(ws.yb, 0, sizeof(float) * (size_t)m_cap * dsh, st);
   prof_begin(m, st, KC_EDGE_MISC, 0);
   // B1 + the first B3 dot: xbar^NL = sigma w_eff;  ubar = c_new (xbar^NL . y^NL)
-  k_xbar_init_dot<<<gridWE, T, 0, st>>>(Mptr, ws.geo, w + P.w_sigma, m->d_weff, D, ws.ylat[NL - 1], m->c_new[NL - 1], ws.xb[0], ws.ub);
+  if (D % 4 == 0 && D / 4 <= 32 && ((D / 4) & (D / 4 - 1)) == 0)
+    k_xbar_init_dot4<<<(unsigned)((m_cap * (D / 4) + T - 1) / T), T, 0, st>>>(Mptr, ws.geo, w + P.w_sigma, m->d_weff, D, ws.ylat[NL - 1],
+                                                                               m->c_new[NL - 1], ws.xb[0], ws.ub);
+  else
+    k_xbar_init_dot<<<gridWE, T, 0, st>>>(Mptr, ws.geo, w + P.w_sigma, m->d_weff, D, ws.ylat[NL - 1], m->c_new[NL - 1], ws.xb[0], ws.ub);
   m->launches += 1;
   prof_end(m, st);
   int xcur = 0, vcur = 0;
@@ -400,8 +404,7 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
     float* wbar = (L == 1) ? ws.wb + nsc : ws.wb;
     const int ldwb = (L == 1) ? 2 * nsc : nsc;
     prof_begin(m, st, KC_GAMMABAR, 0);
-    k_gammabar<<<(unsigned)na, 128, (size_t)(n * dsh + 16) * sizeof(float), st>>>(ws.rowptr_c, ws.geo, ws.ge, ws.wenv[L - 1], ldw_env, n,
-                                                                                  hp.lmax, inv_sqrt_navg, wbar, ldwb, ws.yb, na);
+    launch_gammabar(ws.rowptr_c, ws.geo, ws.ge, ws.wenv[L - 1], ldw_env, n, hp.lmax, inv_sqrt_navg, wbar, ldwb, ws.yb, na, st);
     prof_end(m, st);
     m->launches += 1;
     if (L >= 2) {   // B7: xbar^{L-1} += W_env^T wbar
