@@ -40,6 +40,8 @@ __device__ __forceinline__ float tf32_rna(float x) {
   return __uint_as_float(r);
 }
 
+__device__ __forceinline__ float tf32_trunc(float x) { return __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
+
 // K-major, no swizzle: start address, LBO (k direction) and SBO (row-group direction) in 16-byte units; version 1 (sm_100)
 __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
   uint64_t d = 0;
@@ -556,7 +558,9 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
 #pragma unroll
       for (int qq = 0; qq < 2; ++qq) {
         float4 hi, lo;
-        hi.x = tf32_rna(v[4 * qq]); hi.y = tf32_rna(v[4 * qq + 1]); hi.z = tf32_rna(v[4 * qq + 2]); hi.w = tf32_rna(v[4 * qq + 3]);
+        // hi = the 19 bits the tensor core reads (truncation: one instruction instead of the four of the emulated cvt.rna);
+        // lo = v - hi is exact in fp32 and |lo| < 2^-10 |v|, so hi*hi + hi*lo + lo*hi still carries ~2^-20 per product
+        hi.x = tf32_trunc(v[4 * qq]); hi.y = tf32_trunc(v[4 * qq + 1]); hi.z = tf32_trunc(v[4 * qq + 2]); hi.w = tf32_trunc(v[4 * qq + 3]);
         lo.x = v[4 * qq] - hi.x; lo.y = v[4 * qq + 1] - hi.y; lo.z = v[4 * qq + 2] - hi.z; lo.w = v[4 * qq + 3] - hi.w;
         *reinterpret_cast<float4*>(Ahi + off_row + (half * 2 + qq) * 32) = hi;
         *reinterpret_cast<float4*>(Alo + off_row + (half * 2 + qq) * 32) = lo;
