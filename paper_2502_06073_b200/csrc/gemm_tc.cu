@@ -30,7 +30,7 @@
 namespace allegro {
 namespace {
 
-constexpr int TC_M = 128, TC_KC = 16, TC_T = 256, TC_NMAX = 128;
+constexpr int TC_M = 128, TC_KC = 16, TC_T = 256, TC_NMAX = 256;   // one CTA: 128 rows x up to 256 columns (256 TMEM columns)
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -202,7 +202,7 @@ __global__ void __launch_bounds__(TC_T) k_gemm_tc(GemmArgs a, const float* __res
         for (int e = 0; e < 4; ++e) v[e] *= ascale;
       }
       float4 hi, lo;
-      hi.x = tf32_rna(v[0]); hi.y = tf32_rna(v[1]); hi.z = tf32_rna(v[2]); hi.w = tf32_rna(v[3]);
+      hi.x = tf32_trunc(v[0]); hi.y = tf32_trunc(v[1]); hi.z = tf32_trunc(v[2]); hi.w = tf32_trunc(v[3]);   // see k_gemm_chain
       lo.x = v[0] - hi.x; lo.y = v[1] - hi.y; lo.z = v[2] - hi.z; lo.w = v[3] - hi.w;
       *reinterpret_cast<float4*>(Ahi + off_row + q * 32) = hi;
       *reinterpret_cast<float4*>(Alo + off_row + q * 32) = lo;
@@ -326,7 +326,7 @@ namespace allegro {
 namespace {
 
 static_assert(true, "");
-constexpr int CH_MAX = 4, CH_NB = 4, CH_KMAX = 128, CH_T = TC_T + 64;   // 8 compute warps + weight-loader warp + MMA-issuer warp
+constexpr int CH_MAX = 4, CH_NB = 4, CH_KMAX = 128, CH_NMAX = 128, CH_T = TC_T + 64;   // 8 compute warps + weight-loader warp + MMA-issuer warp
 
 struct ChainArgs {
   int n;
@@ -438,7 +438,7 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
   const int64_t row0 = (int64_t)blockIdx.x * TC_M;
   if (row0 >= M) return;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  constexpr uint32_t a_floats = TC_M * TC_KC, slot_floats = 2 * TC_NMAX * TC_KC;
+  constexpr uint32_t a_floats = TC_M * TC_KC, slot_floats = 2 * CH_NMAX * TC_KC;
   float* As = reinterpret_cast<float*>(smem_raw);          // [2][hi | lo]
   float* Bs = As + 2 * 2 * a_floats;                        // [CH_NB][hi | lo]
 
@@ -654,7 +654,7 @@ bool launch_gemm_chain(Model* m, const GemmArgs* stages, int n_stages, int64_t m
   for (int s = 0; s < n_stages; ++s) {
     const GemmArgs& a = stages[s];
     const int K = a.K0 + a.K1;
-    if (K > CH_KMAX || a.N > TC_NMAX) return false;
+    if (K > CH_KMAX || a.N > CH_NMAX) return false;
     if (s > 0 && (a.K1 != 0 || a.K0 != stages[s - 1].N)) return false;
     bool vec_ok = (a.N % 4 == 0) && (a.ldc % 4 == 0) && al(a.C);
     if (a.C2) vec_ok = vec_ok && (a.ldc2 % 4 == 0) && al(a.C2);
@@ -691,7 +691,7 @@ bool launch_gemm_chain(Model* m, const GemmArgs* stages, int n_stages, int64_t m
     work += 2.0 * stages[s].N * (stages[s].K0 + stages[s].K1);
   }
   (void)nmax;
-  const size_t smem = (size_t)(2 * 2 * TC_M * TC_KC + CH_NB * 2 * TC_NMAX * TC_KC) * sizeof(float);   // 96 KB: two CTAs per SM
+  const size_t smem = (size_t)(2 * 2 * TC_M * TC_KC + CH_NB * 2 * CH_NMAX * TC_KC) * sizeof(float);   // 96 KB: two CTAs per SM
   static bool attr_set = false;
   if (!attr_set) { cudaFuncSetAttribute(k_gemm_chain, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_set = true; }
   prof_begin(m, st, KC_GEMM, work);
