@@ -114,10 +114,11 @@ __global__ void k_pack_w(const float* __restrict__ W, int ldw, int wtrans, int N
 }
 
 // smem per stage: A_hi | A_lo (128 x 16 fp32 each = 8 KB) | B_hi | B_lo (Nt x 16 fp32 each)
-__global__ void __launch_bounds__(TC_T) k_gemm_tc(GemmArgs a, const float* __restrict__ Bp, int Npad, int Kpad, int tmem_cols, int vec_ok) {
+__global__ void __launch_bounds__(TC_T + 32) k_gemm_tc(GemmArgs a, const float* __restrict__ Bp, int Npad, int Kpad, int tmem_cols, int vec_ok) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t mbar_mma[2];
   __shared__ __align__(8) uint64_t mbar_b[2];
+  __shared__ __align__(8) uint64_t mbar_staged[2];         // A staging buffer written by the 8 compute warps
   __shared__ uint32_t tmem_base_s;
   const int64_t M = *a.Mptr * a.m_mul;
   const int64_t row0 = (int64_t)blockIdx.x * TC_M;
@@ -139,6 +140,7 @@ __global__ void __launch_bounds__(TC_T) k_gemm_tc(GemmArgs a, const float* __res
   if (tid == 0) {
     mbar_init(&mbar_mma[0], 1); mbar_init(&mbar_mma[1], 1);
     mbar_init(&mbar_b[0], 1); mbar_init(&mbar_b[1], 1);
+    mbar_init(&mbar_staged[0], 8); mbar_init(&mbar_staged[1], 8);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -148,6 +150,36 @@ __global__ void __launch_bounds__(TC_T) k_gemm_tc(GemmArgs a, const float* __res
   // instruction descriptor: D fp32 (bit 4), A/B tf32 (2 at bits 7 and 10), both K-major, N>>3 at bit 17, M>>4 at bit 24
   const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(Nt >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24);
 
+  if (warp == 8) {
+    // weight loader + MMA issuer (one thread): the compute warps never wait behind the tensor-core queue
+    if (lane == 0) {
+      for (int c = 0; c < nchunks; ++c) {
+        const int b = c & 1;
+        if (c >= 2) mbar_wait(&mbar_mma[b], (uint32_t)(((c >> 1) - 1) & 1));   // slice c-2 done: stage b (A and B) is free
+        uint8_t* st = smem_raw + (size_t)b * stage_bytes;
+        float* Bhi = reinterpret_cast<float*>(st + 2 * a_bytes);
+        bulk_g2s(Bhi, Bt + (int64_t)c * (2 * Nt * TC_KC), 2 * b_bytes, &mbar_b[b]);
+        mbar_wait(&mbar_staged[b], (uint32_t)((c >> 1) & 1));
+        mbar_wait(&mbar_b[b], (uint32_t)((c >> 1) & 1));
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const uint32_t sa_hi = smem_u32(st), sa_lo = sa_hi + a_bytes, sb_hi = smem_u32(Bhi), sb_lo = sb_hi + b_bytes;
+        constexpr uint32_t sbo = (TC_KC / 4) * 128;                   // bytes between 8-row groups
+#pragma unroll
+        for (int ks = 0; ks < TC_KC / 8; ++ks) {
+          const uint32_t koff = ks * 256;                              // two 128-byte k-chunks per K=8 step
+          const uint64_t dAh = umma_desc(sa_hi + koff, 128, sbo), dAl = umma_desc(sa_lo + koff, 128, sbo);
+          const uint64_t dBh = umma_desc(sb_hi + koff, 128, sbo), dBl = umma_desc(sb_lo + koff, 128, sbo);
+          umma_tf32(tmem_d, dAl, dBh, idesc, (c > 0 || ks > 0) ? 1u : 0u);   // small terms first
+          umma_tf32(tmem_d, dAh, dBl, idesc, 1u);
+          umma_tf32(tmem_d, dAh, dBh, idesc, 1u);
+        }
+        umma_commit(&mbar_mma[b]);
+      }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    return;
+  }
   const int r = tid & 127, qh = tid >> 7;              // this thread stages row r, k-quads 2*qh and 2*qh+1 of each slice
   const bool arow_ok = row0 + r < M;
   const int64_t arow = a.amap_d3 ? ((row0 + r) / a.amap_d3) * a.amap_od + a.amap_off + (row0 + r) % a.amap_d3 : row0 + r;
@@ -188,8 +220,6 @@ __global__ void __launch_bounds__(TC_T) k_gemm_tc(GemmArgs a, const float* __res
     uint8_t* st = smem_raw + (size_t)b * stage_bytes;
     float* Ahi = reinterpret_cast<float*>(st);
     float* Alo = reinterpret_cast<float*>(st + a_bytes);
-    float* Bhi = reinterpret_cast<float*>(st + 2 * a_bytes);
-    if (tid == 0) bulk_g2s(Bhi, Bt + (int64_t)c * (2 * Nt * TC_KC), 2 * b_bytes, &mbar_b[b]);
 #pragma unroll
     for (int qq = 0; qq < 2; ++qq) {
       const int q = qh * 2 + qq;
@@ -212,23 +242,8 @@ __global__ void __launch_bounds__(TC_T) k_gemm_tc(GemmArgs a, const float* __res
 #pragma unroll
       for (int e = 0; e < 4; ++e) vcur[qq][e] = vnext[qq][e];
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy smem writes -> visible to the tensor core
-    __syncthreads();
-    if (tid == 0) {
-      mbar_wait(&mbar_b[b], (uint32_t)((c >> 1) & 1));             // the weight block of this slice has landed
-      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-      const uint32_t sa_hi = smem_u32(Ahi), sa_lo = smem_u32(Alo), sb_hi = smem_u32(Bhi), sb_lo = sb_hi + b_bytes;
-      constexpr uint32_t sbo = (TC_KC / 4) * 128;                   // bytes between 8-row groups
-#pragma unroll
-      for (int ks = 0; ks < TC_KC / 8; ++ks) {
-        const uint32_t koff = ks * 256;                              // two 128-byte k-chunks per K=8 step
-        const uint64_t dAh = umma_desc(sa_hi + koff, 128, sbo), dAl = umma_desc(sa_lo + koff, 128, sbo);
-        const uint64_t dBh = umma_desc(sb_hi + koff, 128, sbo), dBl = umma_desc(sb_lo + koff, 128, sbo);
-        umma_tf32(tmem_d, dAl, dBh, idesc, (c > 0 || ks > 0) ? 1u : 0u);   // small terms first
-        umma_tf32(tmem_d, dAh, dBl, idesc, 1u);
-        umma_tf32(tmem_d, dAh, dBh, idesc, 1u);
-      }
-      umma_commit(&mbar_mma[b]);
-    }
+    __syncwarp();
+    if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(&mbar_staged[b])) : "memory");
   }
   {   // all slices issued: wait for the last commit (commits complete in order)
     const int c = nchunks - 1;
@@ -308,7 +323,7 @@ void launch_gemm_tc(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st)
   if (a.epi == EPI_SPLIT_RES) vec_ok = vec_ok && (a.split % 4 == 0);
   dim3 grid((unsigned)((m_cap + TC_M - 1) / TC_M), (unsigned)((Npad + TC_NMAX - 1) / TC_NMAX));
   prof_begin(m, st, KC_GEMM, 2.0 * a.N * K);
-  k_gemm_tc<<<grid, TC_T, smem, st>>>(a, Bp, Npad, Kpad, tmem_cols, vec_ok);
+  k_gemm_tc<<<grid, TC_T + 32, smem, st>>>(a, Bp, Npad, Kpad, tmem_cols, vec_ok);
   prof_end(m, st);
   m->launches += 1;
 }
