@@ -243,58 +243,6 @@ inline void launch_gammabar(const int64_t* rowptr_c, const float* geo, const flo
   }
 }
 
-// B8: wbar_init[e,l,c] = sum_m Vbar0[e,lm,c] Y_lm;  Ybar[e,lm] += sum_c winit[e,l,c] Vbar0[e,lm,c].  One warp per edge,
-// lanes over channels (contiguous).
-__global__ void k_init_bwd(const int64_t* __restrict__ Mptr, const float* __restrict__ geo, const float* __restrict__ vbar0,
-                           const float* __restrict__ winit, int ldwi, int n, int lmax, float* __restrict__ wbar, int ldwb,
-                           float* __restrict__ ybar) {
-  const int lane = threadIdx.x & 31;
-  const int64_t e = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  if (e >= *Mptr) return;
-  const int dsh = (lmax + 1) * (lmax + 1);
-  float Y[16], yb[16];
-  const float* gq = geo + e * GEO_W;
-  sph_harm_rt(lmax, gq[0], gq[1], gq[2], Y);
-#pragma unroll
-  for (int q = 0; q < 16; ++q) yb[q] = 0.f;
-  for (int c = lane; c < n; c += 32) {
-    const float* vb = vbar0 + e * dsh * n + c;
-#pragma unroll
-    for (int l = 0; l < 4; ++l) {
-      if (l <= lmax) {
-        const float wi = winit[e * ldwi + l * n + c];
-        float s = 0.f;
-#pragma unroll
-        for (int mm = 0; mm < 2 * l + 1; ++mm) {
-          const float v = vb[(l * l + mm) * n];
-          s = fmaf(v, Y[l * l + mm], s);
-          yb[l * l + mm] = fmaf(wi, v, yb[l * l + mm]);
-        }
-        wbar[e * ldwb + l * n + c] = s;
-      }
-    }
-  }
-#pragma unroll
-  for (int q = 0; q < 16; ++q) {
-    if (q < dsh) {
-      float v = yb[q];
-#pragma unroll
-      for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
-      if (lane == 0) ybar[e * dsh + q] += v;
-    }
-  }
-}
-
-// B1: xbar^{NL}[e, :] = sigma_{Z_i} * w_eff  (the edge-energy chain has no non-linearity: PAPER.md:93)
-__global__ void k_xbar_init(const int64_t* __restrict__ Mptr, const float* __restrict__ geo, const float* __restrict__ sigma,
-                            const float* __restrict__ weff, int D, float* __restrict__ xbar) {
-  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const int64_t e = idx / D;
-  if (e >= *Mptr) return;
-  const int d = (int)(idx - e * D);
-  xbar[idx] = sigma[__float_as_int(geo[e * GEO_W + 6])] * weff[d];
-}
-
 // active-edge counter of a force call, summed over its atom chunks
 __global__ void k_add_count(const int64_t* __restrict__ cnt, int64_t* __restrict__ total) { *total += *cnt; }
 
