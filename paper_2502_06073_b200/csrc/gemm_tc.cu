@@ -406,36 +406,43 @@ __device__ __forceinline__ void tmem_ld8(uint32_t taddr, float* v) {
 }
 
 // A warp owns 32 rows; each thread computes 16 consecutive columns of its own row.  Global traffic goes through a
-// per-warp shared-memory tile [32][WT_LD] so that one instruction touches 8 rows x 64 contiguous bytes (full sectors)
-// instead of 32 rows x 16 bytes.
-constexpr int WT_LD = 20;
+// per-warp shared-memory tile so that one instruction touches 8 rows x 64 contiguous bytes (full sectors) instead of
+// 32 rows x 16 bytes.  The tile is [32][16] floats with the 16-byte chunk index XOR-swizzled by (row >> 1) & 3: the
+// row-per-lane side (8 lanes = 8 rows, one chunk each) and the transposed side (8 lanes = 2 rows x 4 chunks) are both free of
+// bank conflicts (a padded 20-float row is not: rows r and r+1 of the transposed side overlap by four banks).
+constexpr int WT_LD = 16;
+__device__ __forceinline__ int wt_off(int r, int chunk) { return r * WT_LD + 4 * (chunk ^ ((r >> 1) & 3)); }
 __device__ __forceinline__ void warp_tile_store(float* tile, const float4 (&o)[4], int lane, float* C, int ld, int64_t rbase, int64_t M,
                                                 int col0, int N) {
 #pragma unroll
-  for (int j = 0; j < 4; ++j) *reinterpret_cast<float4*>(tile + lane * WT_LD + 4 * j) = o[j];
+  for (int j = 0; j < 4; ++j) *reinterpret_cast<float4*>(tile + wt_off(lane, j)) = o[j];
   __syncwarp();
   const int cq = (lane & 3) * 4;
+  float4 t[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) t[i] = *reinterpret_cast<const float4*>(tile + wt_off(i * 8 + (lane >> 2), lane & 3));
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
     const int r = i * 8 + (lane >> 2);
-    const float4 t = *reinterpret_cast<const float4*>(tile + r * WT_LD + cq);
-    if (rbase + r < M && col0 + cq < N) *reinterpret_cast<float4*>(C + (rbase + r) * ld + col0 + cq) = t;
+    if (rbase + r < M && col0 + cq < N) *reinterpret_cast<float4*>(C + (rbase + r) * ld + col0 + cq) = t[i];
   }
   __syncwarp();
 }
 __device__ __forceinline__ void warp_tile_load(float* tile, float4 (&x)[4], int lane, const float* A, int ld, int64_t rbase, int64_t M,
                                                int col0, int N) {
   const int cq = (lane & 3) * 4;
+  float4 t[4];
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
     const int r = i * 8 + (lane >> 2);
-    float4 t = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (rbase + r < M && col0 + cq < N) t = *reinterpret_cast<const float4*>(A + (rbase + r) * ld + col0 + cq);
-    *reinterpret_cast<float4*>(tile + r * WT_LD + cq) = t;
+    t[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (rbase + r < M && col0 + cq < N) t[i] = *reinterpret_cast<const float4*>(A + (rbase + r) * ld + col0 + cq);
   }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) *reinterpret_cast<float4*>(tile + wt_off(i * 8 + (lane >> 2), lane & 3)) = t[i];
   __syncwarp();
 #pragma unroll
-  for (int j = 0; j < 4; ++j) x[j] = *reinterpret_cast<const float4*>(tile + lane * WT_LD + 4 * j);
+  for (int j = 0; j < 4; ++j) x[j] = *reinterpret_cast<const float4*>(tile + wt_off(lane, j));
   __syncwarp();
 }
 
@@ -525,7 +532,7 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
   const uint32_t lane_addr = (uint32_t)(quad * 32) << 16;
   const int64_t row = row0 + erow, rbase = row0 + quad * 32;
   const bool row_ok = row < M;
-  float* wtile = As + warp * (32 * WT_LD);                 // 640 floats per warp inside the 8192-float staging area
+  float* wtile = As + warp * (32 * WT_LD);                 // 512 floats per warp inside the 8192-float staging area
   float u = 0.f; int zi = 0, zj = 0;
   if (row_ok) {
     const float* gq = ca.st[0].geo + row * GEO_W;
