@@ -367,29 +367,6 @@ __global__ void k_transpose_wg(const float* __restrict__ Wg, int ldwg, int S, in
 __device__ __forceinline__ bool epi_needs_aux(const GemmArgs& a, int n) {
   return a.epi == EPI_RESIDUAL || a.epi == EPI_DSILU || a.epi == EPI_ACCUM || (a.epi == EPI_SPLIT_RES && n < a.split);
 }
-// epilogue arithmetic of gemm_epi4 without the memory traffic: o1 -> C, o2 -> C2, pass -> next stage
-struct EpiOut { float4 o1, o2, pass; };
-__device__ __forceinline__ EpiOut chain_math(const GemmArgs& a, int n, float4 v, float u, float4 x, float4 gth) {
-  EpiOut r;
-  r.o1 = v; r.o2 = v; r.pass = v;
-  switch (a.epi) {
-    case EPI_GATHER2: v.x += gth.x; v.y += gth.y; v.z += gth.z; v.w += gth.w; r.o1 = v; r.pass = v; break;
-    case EPI_Y_X: r.o2 = make_float4(u * v.x, u * v.y, u * v.z, u * v.w); r.pass = r.o2; break;
-    case EPI_RESIDUAL: {
-      const float cu = a.c_new * u;
-      r.o2 = make_float4(a.c_old * x.x + cu * v.x, a.c_old * x.y + cu * v.y, a.c_old * x.z + cu * v.z, a.c_old * x.w + cu * v.w);
-      r.pass = r.o2;
-    } break;
-    case EPI_DSILU: r.o1 = make_float4(v.x * dsilu_f(x.x), v.y * dsilu_f(x.y), v.z * dsilu_f(x.z), v.w * dsilu_f(x.w)); r.pass = r.o1; break;
-    case EPI_ACCUM: r.o1 = make_float4(x.x + v.x, x.y + v.y, x.z + v.z, x.w + v.w); r.pass = r.o1; break;
-    case EPI_SPLIT_RES:
-      if (n < a.split) r.o1 = make_float4(a.c_old * x.x + v.x, a.c_old * x.y + v.y, a.c_old * x.z + v.z, a.c_old * x.w + v.w);
-      break;
-    default: break;
-  }
-  return r;
-}
-
 __device__ __forceinline__ void tmem_st4(uint32_t taddr, float4 x) {
   asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" ::"r"(taddr), "r"(__float_as_uint(x.x)),
                "r"(__float_as_uint(x.y)), "r"(__float_as_uint(x.z)), "r"(__float_as_uint(x.w))
@@ -567,8 +544,6 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
   for (int s = 0; s < ca.n; ++s) {
     const GemmArgs& a = ca.st[s];
     const int Nt = ca.Npad[s], nchunks = ca.Kpad[s] / TC_KC;
-    const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(Nt >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24);
-    const uint32_t b_bytes = (uint32_t)Nt * TC_KC * 4;
 #pragma unroll 1
     for (int c = 0; c < nchunks; ++c) {
       const int g = gc + c, b = g & 1;
@@ -607,7 +582,7 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
     float dacc = 0.f;
 #pragma unroll 1
     for (int n0 = half * 16; n0 < Nt; n0 += 32) {
-      float4 x[4], o1[4], o2[4], yd[4];
+      float4 x[4], o1[4], yd[4];
       if (a.dot_out && !a.dotv) warp_tile_load(wtile, yd, lane, a.dotB, a.lddot, rbase, M, n0, a.N);
 #pragma unroll
       for (int j = 0; j < 4; ++j) x[j] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -617,32 +592,102 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
       }
       float v[16];
       tmem_ld16(tmem_d + lane_addr + (uint32_t)n0, v);
+      // The epilogue kind is resolved once per 16-column step (not per 4-column group), so that each phase below is one
+      // basic block over all 16 values and the scheduler can overlap their dependency chains.
+      float4 p[4];                                           // what the next stage / the row dot product consumes
+#define CH_V(j) make_float4(v[4 * (j)], v[4 * (j) + 1], v[4 * (j) + 2], v[4 * (j) + 3])
+      switch (a.epi) {
+        case EPI_GATHER2: {
+          const float* g1p = ca.WgT[s] + (int64_t)zi * a.N;
+          const float* g2p = ca.WgT[s] + (int64_t)(a.S + zj) * a.N;
 #pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        const int n = n0 + j * 4;
-        float4 gth = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (a.epi == EPI_GATHER2 && n < a.N) {
-          const float4 g1 = *reinterpret_cast<const float4*>(ca.WgT[s] + (int64_t)zi * a.N + n);
-          const float4 g2 = *reinterpret_cast<const float4*>(ca.WgT[s] + (int64_t)(a.S + zj) * a.N + n);
-          gth = make_float4(g1.x + g2.x, g1.y + g2.y, g1.z + g2.z, g1.w + g2.w);
-        }
-        EpiOut r = chain_math(a, n, make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]), u, x[j], gth);
-        if (!row_ok || n >= a.N) r.pass = make_float4(0.f, 0.f, 0.f, 0.f);
-        o1[j] = r.o1; o2[j] = r.o2;
-        if (a.dot_out && n < a.N) {
-          const float4 y = a.dotv ? *reinterpret_cast<const float4*>(a.dotv + n) : yd[j];
-          dacc = fmaf(r.pass.x, y.x, fmaf(r.pass.y, y.y, fmaf(r.pass.z, y.z, fmaf(r.pass.w, y.w, dacc))));
-        }
-        if (!last)
-          tmem_st4(tmem_act + lane_addr + (uint32_t)n, make_float4(apply_pro(npro, r.pass.x, nscale), apply_pro(npro, r.pass.y, nscale),
-                                                                  apply_pro(npro, r.pass.z, nscale), apply_pro(npro, r.pass.w, nscale)));
+          for (int j = 0; j < 4; ++j) {
+            const int nn = min(n0 + 4 * j, a.N - 4);          // padded columns read a valid address; they are masked below
+            const float4 g1 = *reinterpret_cast<const float4*>(g1p + nn);
+            const float4 g2 = *reinterpret_cast<const float4*>(g2p + nn);
+            const float4 t = CH_V(j);
+            o1[j] = make_float4(t.x + (g1.x + g2.x), t.y + (g1.y + g2.y), t.z + (g1.z + g2.z), t.w + (g1.w + g2.w));
+            p[j] = o1[j];
+          }
+        } break;
+        case EPI_Y_X:
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const float4 t = CH_V(j);
+            o1[j] = t; p[j] = make_float4(u * t.x, u * t.y, u * t.z, u * t.w);
+          }
+          break;
+        case EPI_RESIDUAL: {
+          const float cu = a.c_new * u;
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const float4 t = CH_V(j);
+            o1[j] = t;
+            p[j] = make_float4(a.c_old * x[j].x + cu * t.x, a.c_old * x[j].y + cu * t.y, a.c_old * x[j].z + cu * t.z, a.c_old * x[j].w + cu * t.w);
+          }
+        } break;
+        case EPI_DSILU:
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const float4 t = CH_V(j);
+            o1[j] = make_float4(t.x * dsilu_f(x[j].x), t.y * dsilu_f(x[j].y), t.z * dsilu_f(x[j].z), t.w * dsilu_f(x[j].w));
+            p[j] = o1[j];
+          }
+          break;
+        case EPI_ACCUM:
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const float4 t = CH_V(j);
+            o1[j] = make_float4(x[j].x + t.x, x[j].y + t.y, x[j].z + t.z, x[j].w + t.w);
+            p[j] = o1[j];
+          }
+          break;
+        case EPI_SPLIT_RES: {
+          const bool res = n0 < a.split;                      // split % 16 == 0: a step lies on one side
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const float4 t = CH_V(j);
+            o1[j] = res ? make_float4(a.c_old * x[j].x + t.x, a.c_old * x[j].y + t.y, a.c_old * x[j].z + t.z, a.c_old * x[j].w + t.w) : t;
+            p[j] = t;
+          }
+        } break;
+        default:
+#pragma unroll
+          for (int j = 0; j < 4; ++j) { o1[j] = CH_V(j); p[j] = o1[j]; }
+          break;
       }
+#undef CH_V
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+        if (!row_ok || n0 + 4 * j >= a.N) p[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (a.dot_out) {
+        if (a.dotv) {
+#pragma unroll
+          for (int j = 0; j < 4; ++j) yd[j] = *reinterpret_cast<const float4*>(a.dotv + min(n0 + 4 * j, a.N - 4));
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+          dacc = fmaf(p[j].x, yd[j].x, fmaf(p[j].y, yd[j].y, fmaf(p[j].z, yd[j].z, fmaf(p[j].w, yd[j].w, dacc))));
+      }
+      if (!last) {   // next stage's prologue applied on the way back to TMEM; p itself is still needed for the C2 store
+        if (npro == PRO_SILU) {
+#pragma unroll
+          for (int j = 0; j < 4; ++j)
+            tmem_st4(tmem_act + lane_addr + (uint32_t)(n0 + 4 * j), make_float4(silu_f(p[j].x), silu_f(p[j].y), silu_f(p[j].z), silu_f(p[j].w)));
+        } else {
+          const float sc = (npro == PRO_SCALE_U) ? nscale : 1.f;
+#pragma unroll
+          for (int j = 0; j < 4; ++j)
+            tmem_st4(tmem_act + lane_addr + (uint32_t)(n0 + 4 * j), make_float4(p[j].x * sc, p[j].y * sc, p[j].z * sc, p[j].w * sc));
+        }
+      }
+      // p is zero outside the valid rows / columns, exactly where the tile store is masked: it serves as the C2 operand
       if (a.epi == EPI_SPLIT_RES && n0 >= a.split) {
-        warp_tile_store(wtile, o2, lane, a.C2, a.ldc2, rbase, M, n0 - a.split, a.N - a.split);
+        warp_tile_store(wtile, o1, lane, a.C2, a.ldc2, rbase, M, n0 - a.split, a.N - a.split);
       } else {
         // the adjoint of a hidden layer is consumed by the next chained stage only: it never goes to global memory
         if (!(a.epi == EPI_DSILU && !last)) warp_tile_store(wtile, o1, lane, a.C, a.ldc, rbase, M, n0, a.epi == EPI_SPLIT_RES ? a.split : a.N);
-        if (two) warp_tile_store(wtile, o2, lane, a.C2, a.ldc2, rbase, M, n0, a.N);
+        if (two) warp_tile_store(wtile, p, lane, a.C2, a.ldc2, rbase, M, n0, a.N);
       }
     }
     if (a.dot_out) {   // the two warps that share a row quadrant combine their halves of the row dot product
