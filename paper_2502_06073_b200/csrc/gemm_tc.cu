@@ -341,7 +341,7 @@ namespace allegro {
 namespace {
 
 static_assert(true, "");
-constexpr int CH_MAX = 4, CH_NB = 4, CH_KMAX = 128, CH_NMAX = 128, CH_T = TC_T + 64;   // 8 compute warps + weight-loader warp + MMA-issuer warp
+constexpr int CH_MAX = 4, CH_NB = 3, CH_KMAX = 128, CH_NMAX = 128, CH_T = TC_T + 64;   // 8 compute warps + weight-loader warp + MMA-issuer warp
 
 struct ChainArgs {
   int n;
@@ -350,12 +350,6 @@ struct ChainArgs {
   const float* WgT[CH_MAX];      // EPI_GATHER2: species columns of W transposed, [2S][N]
   int Npad[CH_MAX], Kpad[CH_MAX];
 };
-
-__device__ __forceinline__ float apply_pro(int pro, float v, float ascale) {
-  if (pro == PRO_SILU) return silu_f(v);
-  if (pro == PRO_SCALE_U) return v * ascale;
-  return v;
-}
 
 __global__ void k_transpose_wg(const float* __restrict__ Wg, int ldwg, int S, int N, float* __restrict__ out) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -405,16 +399,33 @@ __device__ __forceinline__ void warp_tile_store(float* tile, const float4 (&o)[4
   }
   __syncwarp();
 }
-__device__ __forceinline__ void warp_tile_load(float* tile, float4 (&x)[4], int lane, const float* A, int ld, int64_t rbase, int64_t M,
-                                               int col0, int N) {
+// Asynchronous load side: cp.async writes the transposed side of a tile directly (no registers, zero fill outside the valid
+// rows / columns); after cp.async.wait_group + __syncwarp the owner lanes read their rows with warp_tile_read.
+__device__ __forceinline__ void warp_tile_prefetch(float* tile, int lane, const float* A, int ld, int64_t rbase, int64_t M, int col0, int N) {
   const int cq = (lane & 3) * 4;
-  float4 t[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int r = i * 8 + (lane >> 2);
+    const bool ok = rbase + r < M && col0 + cq < N;
+    const float* src = ok ? A + (rbase + r) * ld + col0 + cq : A;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_u32(tile + wt_off(r, lane & 3))), "l"(src), "r"(ok ? 16u : 0u) : "memory");
+  }
+}
+__device__ __forceinline__ void warp_tile_read(const float* tile, float4 (&x)[4], int lane) {
+#pragma unroll
+  for (int j = 0; j < 4; ++j) x[j] = *reinterpret_cast<const float4*>(tile + wt_off(lane, j));
+}
+// load side in two steps, so that the global loads of several row segments can be in flight before the first transposition
+__device__ __forceinline__ void warp_tile_ldg(float4 (&t)[4], int lane, const float* A, int ld, int64_t rbase, int64_t M, int col0, int N) {
+  const int cq = (lane & 3) * 4;
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
     const int r = i * 8 + (lane >> 2);
     t[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     if (rbase + r < M && col0 + cq < N) t[i] = *reinterpret_cast<const float4*>(A + (rbase + r) * ld + col0 + cq);
   }
+}
+__device__ __forceinline__ void warp_tile_xpose(float* tile, const float4 (&t)[4], float4 (&x)[4], int lane) {
 #pragma unroll
   for (int i = 0; i < 4; ++i) *reinterpret_cast<float4*>(tile + wt_off(i * 8 + (lane >> 2), lane & 3)) = t[i];
   __syncwarp();
@@ -422,7 +433,6 @@ __device__ __forceinline__ void warp_tile_load(float* tile, float4 (&x)[4], int 
   for (int j = 0; j < 4; ++j) x[j] = *reinterpret_cast<const float4*>(tile + wt_off(lane, j));
   __syncwarp();
 }
-
 // TMEM: columns [0, 128) accumulator D, columns [128, 256) the activation that feeds the current stage (fp32, prologue
 // already applied).  Shared memory: two 16-deep A staging buffers (hi | lo, canonical layout; reused as the per-warp
 // transposition tiles of the epilogue) and CH_NB weight slots filled by a dedicated loader warp.
@@ -509,7 +519,11 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
   const uint32_t lane_addr = (uint32_t)(quad * 32) << 16;
   const int64_t row = row0 + erow, rbase = row0 + quad * 32;
   const bool row_ok = row < M;
-  float* wtile = As + warp * (32 * WT_LD);                 // 512 floats per warp inside the 8192-float staging area
+  // per-warp tiles: wtile (stores, stage-in) and dtile (prefetched dot operand) inside the A staging area, which is idle during
+  // the epilogues; xtile (prefetched auxiliary rows) behind the weight slots, so that it can be filled during the k loop
+  float* wtile = As + warp * (2 * 32 * WT_LD);
+  float* dtile = wtile + 32 * WT_LD;
+  float* xtile = Bs + CH_NB * slot_floats + warp * (32 * WT_LD);
   float u = 0.f; int zi = 0, zj = 0;
   if (row_ok) {
     const float* gq = ca.st[0].geo + row * GEO_W;
@@ -521,17 +535,33 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
     const int ngrp = ca.Kpad[0] >> 4;
     float ascale = 1.f;
     if (a.pro == PRO_SCALE_U) ascale = a.c_new * u;
-#pragma unroll 1
-    for (int gk = half; gk < ngrp; gk += 2) {
-      const int k0 = gk * 16;
+    auto ldg_grp = [&](float4 (&t)[4], int k0) {
+      if (k0 < a.K0) warp_tile_ldg(t, lane, a.A0, a.lda0, rbase, M, k0, a.K0);
+      else warp_tile_ldg(t, lane, a.A1, a.lda1, rbase, M, k0 - a.K0, a.K1);
+    };
+    auto put_grp = [&](const float4 (&t)[4], int k0) {
       float4 x[4];
-      if (k0 < a.K0) warp_tile_load(wtile, x, lane, a.A0, a.lda0, rbase, M, k0, a.K0);
-      else warp_tile_load(wtile, x, lane, a.A1, a.lda1, rbase, M, k0 - a.K0, a.K1);
+      warp_tile_xpose(wtile, t, x, lane);
+      if (a.pro == PRO_SILU) {
 #pragma unroll
-      for (int j = 0; j < 4; ++j)
-        tmem_st4(tmem_act + lane_addr + (uint32_t)(k0 + 4 * j),
-                 make_float4(apply_pro(a.pro, x[j].x, ascale), apply_pro(a.pro, x[j].y, ascale), apply_pro(a.pro, x[j].z, ascale),
-                             apply_pro(a.pro, x[j].w, ascale)));
+        for (int j = 0; j < 4; ++j) x[j] = make_float4(silu_f(x[j].x), silu_f(x[j].y), silu_f(x[j].z), silu_f(x[j].w));
+      } else {
+        const float sc = (a.pro == PRO_SCALE_U) ? ascale : 1.f;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) x[j] = make_float4(x[j].x * sc, x[j].y * sc, x[j].z * sc, x[j].w * sc);
+      }
+#pragma unroll
+      for (int j = 0; j < 4; ++j) tmem_st4(tmem_act + lane_addr + (uint32_t)(k0 + 4 * j), x[j]);
+    };
+    // two 16-column groups per iteration: both global loads are in flight before the first one is consumed
+#pragma unroll 1
+    for (int gk = half; gk < ngrp; gk += 4) {
+      float4 t0[4], t1[4];
+      const bool second = gk + 2 < ngrp;
+      ldg_grp(t0, gk * 16);
+      if (second) ldg_grp(t1, (gk + 2) * 16);
+      put_grp(t0, gk * 16);
+      if (second) put_grp(t1, (gk + 2) * 16);
     }
     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
   }
@@ -544,6 +574,12 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
   for (int s = 0; s < ca.n; ++s) {
     const GemmArgs& a = ca.st[s];
     const int Nt = ca.Npad[s], nchunks = ca.Kpad[s] / TC_KC;
+    const bool ld_d = a.dot_out && !a.dotv;
+    const float* xsrc = (a.epi == EPI_ACCUM) ? a.C : a.aux;
+    const int ldx = (a.epi == EPI_ACCUM) ? a.ldc : a.ldaux;
+    // auxiliary rows of the first epilogue step: in flight during the whole k loop
+    if (epi_needs_aux(a, half * 16)) warp_tile_prefetch(xtile, lane, xsrc, ldx, rbase, M, half * 16, a.N);
+    asm volatile("cp.async.commit_group;" ::: "memory");
 #pragma unroll 1
     for (int c = 0; c < nchunks; ++c) {
       const int g = gc + c, b = g & 1;
@@ -580,15 +616,25 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
     const float nscale = (!last && npro == PRO_SCALE_U) ? ca.st[s + 1].c_new * u : 1.f;
     const bool two = (a.epi == EPI_Y_X || a.epi == EPI_RESIDUAL);
     float dacc = 0.f;
+    if (ld_d) warp_tile_prefetch(dtile, lane, a.dotB, a.lddot, rbase, M, half * 16, a.N);
+    asm volatile("cp.async.commit_group;" ::: "memory");
 #pragma unroll 1
     for (int n0 = half * 16; n0 < Nt; n0 += 32) {
       float4 x[4], o1[4], yd[4];
-      if (a.dot_out && !a.dotv) warp_tile_load(wtile, yd, lane, a.dotB, a.lddot, rbase, M, n0, a.N);
+      {   // this step's auxiliary row segments were prefetched; the next step's are requested before the arithmetic
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncwarp();
 #pragma unroll
-      for (int j = 0; j < 4; ++j) x[j] = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (epi_needs_aux(a, n0)) {
-        if (a.epi == EPI_ACCUM) warp_tile_load(wtile, x, lane, a.C, a.ldc, rbase, M, n0, a.N);
-        else warp_tile_load(wtile, x, lane, a.aux, a.ldaux, rbase, M, n0, a.N);
+        for (int j = 0; j < 4; ++j) { x[j] = make_float4(0.f, 0.f, 0.f, 0.f); yd[j] = x[j]; }
+        if (ld_d) warp_tile_read(dtile, yd, lane);
+        if (epi_needs_aux(a, n0)) warp_tile_read(xtile, x, lane);
+        __syncwarp();
+        const int n1 = n0 + 32;
+        if (n1 < Nt) {
+          if (ld_d) warp_tile_prefetch(dtile, lane, a.dotB, a.lddot, rbase, M, n1, a.N);
+          if (epi_needs_aux(a, n1)) warp_tile_prefetch(xtile, lane, xsrc, ldx, rbase, M, n1, a.N);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
       }
       float v[16];
       tmem_ld16(tmem_d + lane_addr + (uint32_t)n0, v);
@@ -758,7 +804,8 @@ bool launch_gemm_chain(Model* m, const GemmArgs* stages, int n_stages, int64_t m
     work += 2.0 * stages[s].N * (stages[s].K0 + stages[s].K1);
   }
   (void)nmax;
-  const size_t smem = (size_t)(2 * 2 * TC_M * TC_KC + CH_NB * 2 * CH_NMAX * TC_KC) * sizeof(float);   // 96 KB: two CTAs per SM
+  // A staging 32 KB + CH_NB weight slots 48 KB + one prefetch tile per compute warp 16 KB = 96 KB: two CTAs per SM
+  const size_t smem = (size_t)(2 * 2 * TC_M * TC_KC + CH_NB * 2 * CH_NMAX * TC_KC + 8 * 32 * WT_LD) * sizeof(float);
   static bool attr_set = false;
   if (!attr_set) { cudaFuncSetAttribute(k_gemm_chain, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_set = true; }
   prof_begin(m, st, KC_GEMM, work);
