@@ -333,14 +333,14 @@ void launch_gemm_tc(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st)
 // =============================================================================================================
 // Chained GEMMs: up to CH_MAX dependent linears of one MLP on the same 128-row tile of edges.  The activation never
 // leaves the SM between stages: the epilogue of stage s reads the accumulator from TMEM, applies its fused epilogue
-// (global stores of what the backward pass needs), applies the prologue of stage s+1 and writes the result, split
-// hi/lo, straight into the canonical K-major UMMA layout of the next A operand.  The k loop therefore has no staging
-// work at all: one thread streams the pre-packed weight slices with cp.async.bulk (3 slots) and issues the MMAs.
+// (global stores of what the backward pass needs), applies the prologue of stage s+1 and writes the fp32 result to the
+// activation columns of TMEM; in the k loop the compute warps read it back 16 columns at a time, split it hi/lo and stage
+// it in the canonical K-major UMMA layout, a loader warp streams the pre-packed weight slices with cp.async.bulk
+// (CH_NB slots) and an issuer warp issues the MMAs.  Details above k_gemm_chain and in DESIGN.md section 6.
 // =============================================================================================================
 namespace allegro {
 namespace {
 
-static_assert(true, "");
 constexpr int CH_MAX = 4, CH_NB = 3, CH_KMAX = 128, CH_NMAX = 128, CH_T = TC_T + 64;   // 8 compute warps + weight-loader warp + MMA-issuer warp
 
 struct ChainArgs {
