@@ -264,10 +264,42 @@ __global__ void __launch_bounds__(TC_T + 32) k_gemm_tc(GemmArgs a, const float* 
     tmem_ld16(tmem_d + ((uint32_t)(quad * 32) << 16) + (uint32_t)n0, v);
     if (row < M) {
       if (vec_ok) {
+        const int nb = col0 + n0;
+        const bool aux_kind = a.epi == EPI_DSILU || a.epi == EPI_RESIDUAL || a.epi == EPI_ACCUM || (a.epi == EPI_SPLIT_RES && nb + 16 <= a.split);
+        if (aux_kind) {
+          // the four auxiliary loads of a 16-column step are issued together (one basic block), then the arithmetic, then the
+          // stores: the per-group form waits for one global load at a time (42 % of the warp-state samples of this kernel,
+          // profiles/r1_h_gemm_tc.md).  Columns past N read a clamped valid address and are not stored.
+          const float* xs = (a.epi == EPI_ACCUM) ? a.C + row * a.ldc : a.aux + row * a.ldaux;
+          float4 x[4];
 #pragma unroll
-        for (int j = 0; j < 16; j += 4) {
-          const int n = col0 + n0 + j;
-          if (n < a.N) gemm_epi4(a, row, n, make_float4(v[j], v[j + 1], v[j + 2], v[j + 3]), u, zi, zj);
+          for (int j = 0; j < 4; ++j) x[j] = *reinterpret_cast<const float4*>(xs + min(nb + 4 * j, a.N - 4));
+          float4 o1[4], o2[4];
+          const float cu = a.c_new * u;
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const float4 t = make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]);
+            o1[j] = t; o2[j] = t;
+            if (a.epi == EPI_DSILU) o1[j] = make_float4(t.x * dsilu_f(x[j].x), t.y * dsilu_f(x[j].y), t.z * dsilu_f(x[j].z), t.w * dsilu_f(x[j].w));
+            else if (a.epi == EPI_ACCUM) o1[j] = make_float4(x[j].x + t.x, x[j].y + t.y, x[j].z + t.z, x[j].w + t.w);
+            else if (a.epi == EPI_RESIDUAL)
+              o2[j] = make_float4(a.c_old * x[j].x + cu * t.x, a.c_old * x[j].y + cu * t.y, a.c_old * x[j].z + cu * t.z, a.c_old * x[j].w + cu * t.w);
+            else o1[j] = make_float4(a.c_old * x[j].x + t.x, a.c_old * x[j].y + t.y, a.c_old * x[j].z + t.z, a.c_old * x[j].w + t.w);
+          }
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const int n = nb + 4 * j;
+            if (n < a.N) {
+              *reinterpret_cast<float4*>(a.C + row * a.ldc + n) = o1[j];
+              if (a.epi == EPI_RESIDUAL) *reinterpret_cast<float4*>(a.C2 + row * a.ldc2 + n) = o2[j];
+            }
+          }
+        } else {
+#pragma unroll
+          for (int j = 0; j < 16; j += 4) {
+            const int n = col0 + n0 + j;
+            if (n < a.N) gemm_epi4(a, row, n, make_float4(v[j], v[j + 1], v[j + 2], v[j + 3]), u, zi, zj);
+          }
         }
       } else {
 #pragma unroll
