@@ -126,6 +126,18 @@ int allegro_get_profile(void* h, double* ms, int64_t* launches, double* work, in
 int allegro_debug_coupling(int l1, int l2, int l3, double* out);
 int allegro_debug_num_paths(const allegro_hparams* hp, int layer);
 
+/* Test hooks for the split-fp16 tcgen05 GEMM of the wide linears (csrc/gemm_f16s.cu; PAPER.md:93 / Table 1 MLPs).
+ * allegro_debug_set_precision: 3 (default) = hi*hi + hi*lo + lo*hi, 2 = activations split only, 1 = plain fp16 — the
+ * 1/2-pass kinds exist only for the committed precision study (R4).
+ * allegro_debug_gemm runs one launch of that kernel on caller data:  C[M,N] = epi( pro([A0 | A1]) B ),  B(k,n) = wtrans ?
+ * W[k*ldw+n] : W[n*ldw+k];  pro / epi are the PRO_* / EPI_* codes of csrc/gemm.cuh (0/1/2 and 0..6).  All pointers DEVICE fp32;
+ * A0 / A1 hold rows_cap >= M rows; geo is the [M][8] edge record (u at [4]) or NULL.  Synchronises the stream.
+ * Returns ALLEGRO_ERR_UNSUPPORTED when the shape or alignment is outside what the kernel takes. */
+int allegro_debug_set_precision(void* h, int passes);
+int allegro_debug_gemm(void* h, int64_t M, int64_t rows_cap, const float* A0, int lda0, int K0, const float* A1, int lda1, int K1,
+                       const float* W, int ldw, int wtrans, int N, int pro, int epi, const float* aux, int ldaux, const float* geo,
+                       float* C, int ldc, float* C2, int ldc2, int split, float c_old, float c_new, void* stream);
+
 const char* allegro_last_error(void* h);
 
 #ifdef __cplusplus

@@ -25,7 +25,8 @@ ERR_NAMES = {0: "OK", -1: "INVALID", -2: "UNSUPPORTED", -3: "CUDA", -4: "STALE_L
 EXPORTS = ["allegro_weight_layout", "allegro_create", "allegro_destroy", "allegro_build_neighbors",
            "allegro_energy_forces", "allegro_md_init", "allegro_md_step", "allegro_get_state",
            "allegro_get_neighbors", "allegro_get_stats", "allegro_profile", "allegro_get_profile",
-           "allegro_debug_coupling", "allegro_debug_num_paths", "allegro_last_error"]
+           "allegro_debug_coupling", "allegro_debug_num_paths", "allegro_debug_set_precision", "allegro_debug_gemm",
+           "allegro_last_error"]
 PROFILE_CLASSES = ["gemm", "tp_fwd", "tp_bwd", "gamma", "gammabar", "active_edges", "edge_misc", "neighbor", "md",
                    "force_gather"]
 
@@ -60,6 +61,9 @@ _lib.allegro_profile.argtypes = [_vp, C.c_int]
 _lib.allegro_get_profile.argtypes = [_vp, _vp, _vp, _vp, C.c_int]
 _lib.allegro_debug_coupling.argtypes = [C.c_int, C.c_int, C.c_int, _vp]
 _lib.allegro_debug_num_paths.argtypes = [C.POINTER(HParams), C.c_int]
+_lib.allegro_debug_set_precision.argtypes = [_vp, C.c_int]
+_lib.allegro_debug_gemm.argtypes = [_vp, _i64, _i64, _vp, C.c_int, C.c_int, _vp, C.c_int, C.c_int, _vp, C.c_int, C.c_int, C.c_int,
+                                    C.c_int, C.c_int, _vp, C.c_int, _vp, _vp, C.c_int, _vp, C.c_int, C.c_int, C.c_float, C.c_float, _vp]
 _lib.allegro_last_error.argtypes = [_vp]
 _lib.allegro_last_error.restype = C.c_char_p
 for _n in EXPORTS[:-1]:
@@ -205,6 +209,18 @@ class Allegro:
         if n < 0:
             self._check(n)
         return {PROFILE_CLASSES[k]: dict(ms=float(ms[k]), launches=int(ln[k]), work=float(wk[k])) for k in range(n)}
+
+    def debug_set_precision(self, passes: int):
+        self._check(_lib.allegro_debug_set_precision(self._h, int(passes)))
+
+    def debug_gemm(self, M, rows_cap, A0, K0, W, N, C_out, A1=None, K1=0, wtrans=0, ldw=None, pro=0, epi=0, aux=None, geo=None,
+                   C2=None, split=0, c_old=0.0, c_new=1.0):
+        """One launch of the split-fp16 GEMM kernel on torch CUDA fp32 tensors (row-major, leading dimension = shape[1])."""
+        ld = lambda t: 0 if t is None else int(t.shape[1])
+        self._check(_lib.allegro_debug_gemm(self._h, int(M), int(rows_cap), _ptr(A0), ld(A0), int(K0), _ptr(A1), ld(A1), int(K1),
+                                            _ptr(W), int(ldw if ldw is not None else W.shape[1]), int(wtrans), int(N), int(pro), int(epi),
+                                            _ptr(aux), ld(aux), _ptr(geo), _ptr(C_out), ld(C_out), _ptr(C2), ld(C2), int(split),
+                                            float(c_old), float(c_new), _stream()))
 
     # convenience wrappers (allocation + marshalling only) ---------------------------------------
     def compute(self, pos_np, species_np, cell, skin=0.0, want_atom=False):

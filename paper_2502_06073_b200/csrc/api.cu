@@ -4,6 +4,7 @@
 #include <cstring>
 #include <new>
 
+#include "gemm.cuh"
 #include "model.h"
 #include "tp_gen.cuh"
 
@@ -376,6 +377,36 @@ int allegro_get_profile(void* h, double* ms, int64_t* launches, double* work, in
     if (work) work[k] = m->prof.work[k];
   }
   return KC_COUNT;
+}
+
+int allegro_debug_set_precision(void* h, int passes) {
+  if (!h || passes < 1 || passes > 3) return ALLEGRO_ERR_INVALID;
+  static_cast<Model*>(h)->f16_passes = passes;
+  return ALLEGRO_OK;
+}
+
+int allegro_debug_gemm(void* h, int64_t M, int64_t rows_cap, const float* A0, int lda0, int K0, const float* A1, int lda1, int K1,
+                       const float* W, int ldw, int wtrans, int N, int pro, int epi, const float* aux, int ldaux, const float* geo,
+                       float* C, int ldc, float* C2, int ldc2, int split, float c_old, float c_new, void* stream) {
+  if (!h || !A0 || !W || !C || M < 0 || rows_cap < M) return ALLEGRO_ERR_INVALID;
+  Model* m = static_cast<Model*>(h);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if (int rc = ensure(m, &m->act_total, sizeof(int64_t))) return rc;
+  cudaMemcpyAsync(m->act_total.p, &M, sizeof(int64_t), cudaMemcpyHostToDevice, st);
+  GemmArgs g;
+  g.Mptr = m->act_total.as<int64_t>(); g.geo = geo;
+  g.A0 = A0; g.lda0 = lda0; g.K0 = K0; g.A1 = A1; g.lda1 = lda1; g.K1 = K1;
+  g.W = W; g.ldw = ldw; g.wtrans = wtrans; g.N = N; g.pro = pro; g.epi = epi;
+  g.aux = aux; g.ldaux = ldaux; g.C = C; g.ldc = ldc; g.C2 = C2; g.ldc2 = ldc2; g.split = split; g.c_old = c_old; g.c_new = c_new;
+  const int64_t keep = m->f16_rows_cap;
+  m->f16_rows_cap = rows_cap;
+  const bool ok = launch_gemm_f16s(m, g, M, st);
+  m->f16_rows_cap = keep;
+  cudaError_t e = cudaStreamSynchronize(st);
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail(m, e, "allegro_debug_gemm");
+  if (!ok) { m->err = "allegro_debug_gemm: shape or alignment outside the split-fp16 kernel"; return ALLEGRO_ERR_UNSUPPORTED; }
+  return ALLEGRO_OK;
 }
 
 const char* allegro_last_error(void* h) {

@@ -236,9 +236,17 @@ float* packed_weights(Model* m, const GemmArgs& a, cudaStream_t st, int* Npad, i
 // returns false when the shapes do not fit (caller launches the stages one by one)
 bool launch_gemm_chain(Model* m, const GemmArgs* stages, int n_stages, int64_t m_cap, cudaStream_t st);
 
+// split-fp16 tcgen05 kernel for the wide linears (gemm_f16s.cu); false = shape / alignment outside what it takes
+bool launch_gemm_f16s(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st);
+// species columns of the first two-body matrix, transposed once and cached: WgT[z][n] = Wg[n * ldwg + z], z < 2S (gemm_tc.cu)
+const float* transposed_species_columns(Model* m, const GemmArgs& a, cudaStream_t st);
+
 inline void launch_gemm(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st) {
   if (m_cap <= 0) return;
-  if (m->use_tc) { launch_gemm_tc(m, a, m_cap, st); return; }
+  if (m->use_tc) {
+    if (!launch_gemm_f16s(m, a, m_cap, st)) launch_gemm_tc(m, a, m_cap, st);
+    return;
+  }
   dim3 grid((unsigned)((m_cap + GM - 1) / GM), (unsigned)((a.N + GN - 1) / GN));
   prof_begin(m, st, KC_GEMM, 2.0 * a.N * (a.K0 + a.K1));
   k_gemm<<<grid, GT, 0, st>>>(a);

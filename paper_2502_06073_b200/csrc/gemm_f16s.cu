@@ -1,0 +1,515 @@
+// gemm_f16s.cu — the wide edge-by-width GEMMs (latent / two-body MLPs, W_init / W_env, channel mixing and their transposes;
+// PAPER.md:93, Table 1) on tcgen05 with a split-fp16 operand format, for the networks whose widths exceed the chained kernel
+// of gemm_tc.cu (BASELINE.json configs 2 and 3).  Same contract as k_gemm (gemm.cuh):  C = epi( pro(A) B ).
+//
+// Precision ("only in a precision that stays inside the stated tolerance", north_star): every operand x is split as
+//   x = hi + lo / 2048,   hi = fp16(x),  lo = fp16((x - hi) * 2048)      (2 x 11 significant bits, the scaling keeps lo normal)
+// and the product is formed from three kind::f16 passes with fp32 accumulation in two TMEM accumulators,
+//   D0 = A_hi B_hi,   D1 = A_hi B_lo + A_lo B_hi,   A B ~= D0 + D1 / 2048          (lo x lo ~ 2^-24 dropped)
+// i.e. the error-corrected split of Ootomo & Yokota (2022), restated.  It carries ~2^-22 per product like the 3 x TF32 split of
+// gemm_tc.cu at twice the tensor-pipe rate and half the operand bytes.  |x| >= 65520 overflows fp16 (the force call then ends
+// with ALLEGRO_ERR_NONFINITE); R4 has the measured error table for 1, 2 and 3 passes.
+//
+// One persistent CTA per SM (21 warps), tiles of 128 rows x up to 256 columns, K in stages of 32:
+//   * 2 warps issue the TMA loads of the raw fp32 A stage (128 x 32, SWIZZLE_128B tensor map; rows past the list are
+//     zero-filled by the TMA unit), 2 warps the bulk copies of the pre-packed weight stage (one contiguous hi|lo block per
+//     stage): a bulk operation costs its issuing thread ~330 ns whatever its size (profiles/r2_a_probes.md), so the two
+//     streams alternate between two threads each;
+//   * 8 converter warps read the raw stage (conflict-free: one row per lane of a quarter-warp), apply the prologue (SiLU or
+//     the per-row c_new u scale), split hi / lo and write the canonical K-major UMMA tiles;
+//   * 1 thread issues the 2 x 3 tcgen05.mma.kind::f16 (M = 128, N <= 256, K = 16) of a stage and commits them to the stage
+//     barrier, which frees the converted A tile and the weight slot;
+//   * 8 epilogue warps (two per TMEM lane quadrant) read D0 / D1 with tcgen05.ld, combine, apply the fused epilogue and move
+//     rows through per-warp swizzled tiles so that every global access covers full 32-byte sectors.
+// D0 + D1 take all 512 TMEM columns for a 256-column tile, so the accumulators are single-buffered: the loads and the
+// conversions of the next tile run during the epilogue, the tensor pipe waits for it.
+#include <cuda.h>
+#include <cuda_fp16.h>
+
+#include <algorithm>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+
+#include "gemm.cuh"
+#include "tc_common.cuh"
+
+namespace allegro {
+namespace {
+
+constexpr int F_M = 128, F_KS = 32, F_NT = 256, F_S = 3;
+constexpr int F_PROD = 4, F_CVT = 8, F_EPI = 8;
+constexpr int F_W_MMA = F_PROD, F_W_CVT0 = F_PROD + 1, F_W_EPI0 = F_W_CVT0 + F_CVT;
+constexpr int F_T = (F_PROD + 1 + F_CVT + F_EPI) * 32;                 // 672 threads
+constexpr uint32_t F_RAW_BYTES = F_M * F_KS * 4;                        // fp32 A stage as loaded
+constexpr uint32_t F_CVT_BYTES = F_M * F_KS * 2;                        // one of A_hi / A_lo
+constexpr uint32_t F_BMAX_BYTES = F_NT * F_KS * 2;                      // one of B_hi / B_lo at 256 columns
+constexpr uint32_t F_OFF_CVT = F_RAW_BYTES, F_OFF_B = F_RAW_BYTES + 2 * F_CVT_BYTES;
+constexpr uint32_t F_STAGE_BYTES = F_OFF_B + 2 * F_BMAX_BYTES;          // 64 KB
+constexpr uint32_t F_TILE_FLOATS = 32 * WT_LD;                          // per-warp transposition tile
+constexpr size_t F_SMEM = (size_t)F_S * F_STAGE_BYTES + (size_t)F_EPI * 2 * F_TILE_FLOATS * 4 + 1024;
+constexpr float F_LO_SCALE = 2048.0f, F_LO_INV = 1.0f / 2048.0f;
+
+struct FArgs {
+  GemmArgs a;
+  const uint8_t* Bp;        // packed hi | lo weight stages per column tile
+  const float* WgT;         // EPI_GATHER2: transposed species columns [2S][N]
+  int Npad, Kpad, n_nt;     // N padded to 16, K to 32, number of column tiles
+  int nk0, nk;              // K stages that read A0, total
+  int passes;               // 3 = full split, 2 = activations split only, 1 = plain fp16 (precision study)
+};
+
+__device__ __forceinline__ void mbar_wait_b(uint64_t* bar, uint32_t parity) {
+  // bounded: a protocol error ends in a trap (sticky CUDA error) instead of a hung GPU
+  uint32_t done = 0;
+  for (uint32_t it = 0; !done; ++it) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done)
+        : "r"(smem_u32(bar)), "r"(parity), "r"(1000u)
+        : "memory");
+    if (it > (1u << 22)) __trap();
+  }
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* tm, int c0, int c1, uint64_t* bar) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(smem_u32(dst)),
+               "l"(tm), "r"(c0), "r"(c1), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void umma_f16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate));
+}
+// x -> (hi, lo): hi = fp16(x), lo = fp16((x - hi) * 2048)
+__device__ __forceinline__ void split8(const float (&v)[8], uint4& hi, uint4& lo) {
+  uint32_t h[4], l[4];
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const __half2 hh = __floats2half2_rn(v[2 * j], v[2 * j + 1]);
+    const float2 hf = __half22float2(hh);
+    const __half2 ll = __floats2half2_rn((v[2 * j] - hf.x) * F_LO_SCALE, (v[2 * j + 1] - hf.y) * F_LO_SCALE);
+    h[j] = *reinterpret_cast<const uint32_t*>(&hh);
+    l[j] = *reinterpret_cast<const uint32_t*>(&ll);
+  }
+  hi = make_uint4(h[0], h[1], h[2], h[3]);
+  lo = make_uint4(l[0], l[1], l[2], l[3]);
+}
+
+// packed B: per column tile t (n0 = 256 t, Nt columns), per K stage c: [hi: Nt x 32 fp16 | lo: Nt x 32 fp16], each in the canonical
+// K-major no-swizzle UMMA layout [n/8][k/8][n%8][k%8] (core matrix = 8 rows x 16 bytes; LBO 128 B, SBO 512 B)
+__global__ void k_pack_w16(const float* __restrict__ W, int ldw, int wtrans, int N, int K, int Npad, int Kpad, uint8_t* __restrict__ out) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (int64_t)Npad * Kpad) return;
+  const int n = (int)(idx / Kpad), k = (int)(idx - (int64_t)n * Kpad);
+  float v = 0.f;
+  if (n < N && k < K) v = wtrans ? W[(int64_t)k * ldw + n] : W[(int64_t)n * ldw + k];
+  const __half hi = __float2half_rn(v);
+  const __half lo = __float2half_rn((v - __half2float(hi)) * F_LO_SCALE);
+  const int tile = n / F_NT, nl = n - tile * F_NT, Nt = min(Npad - tile * F_NT, F_NT);
+  const int c = k / F_KS, kl = k - c * F_KS;
+  const size_t base = (size_t)tile * F_NT * Kpad * 4 + (size_t)c * Nt * (F_KS * 4);
+  const int off = (nl >> 3) * 512 + (kl >> 3) * 128 + (nl & 7) * 16 + (kl & 7) * 2;
+  *reinterpret_cast<__half*>(out + base + off) = hi;
+  *reinterpret_cast<__half*>(out + base + (size_t)Nt * (F_KS * 2) + off) = lo;
+}
+
+// row r of the GEMM -> row of the C tensor (tp_big.cuh: (edge, m) pairs of one irrep inside [e][comp][c])
+__device__ __forceinline__ int64_t crow(const GemmArgs& a, int64_t r) {
+  return a.cmap_d3 ? (r / a.cmap_d3) * a.cmap_od + a.cmap_off + r % a.cmap_d3 : r;
+}
+// per-warp tile store of 32 rows x 16 columns with the row map applied
+__device__ __forceinline__ void tile_store_map(float* tile, const float4 (&o)[4], int lane, const GemmArgs& a, float* C, int ld, int64_t rbase,
+                                               int64_t M, int col0, int N, bool mapped) {
+#pragma unroll
+  for (int j = 0; j < 4; ++j) *reinterpret_cast<float4*>(tile + wt_off(lane, j)) = o[j];
+  __syncwarp();
+  const int cq = (lane & 3) * 4;
+  float4 t[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) t[i] = *reinterpret_cast<const float4*>(tile + wt_off(i * 8 + (lane >> 2), lane & 3));
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int64_t r = rbase + i * 8 + (lane >> 2);
+    if (r < M && col0 + cq < N) *reinterpret_cast<float4*>(C + (mapped ? crow(a, r) : r) * ld + col0 + cq) = t[i];
+  }
+  __syncwarp();
+}
+
+__global__ void __launch_bounds__(F_T, 1) k_gemm_f16s(const __grid_constant__ FArgs fa, const __grid_constant__ CUtensorMap tmA0,
+                                                       const __grid_constant__ CUtensorMap tmA1) {
+  extern __shared__ uint8_t smem_dyn[];
+  __shared__ __align__(8) uint64_t raw_full[F_S], raw_empty[F_S], cvt_full[F_S], b_full[F_S], mma_done[F_S];
+  __shared__ __align__(8) uint64_t acc_full, acc_empty;
+  __shared__ uint32_t tmem_base_s;
+  const GemmArgs& a = fa.a;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  uint8_t* smem = smem_dyn + ((1024u - (smem_u32(smem_dyn) & 1023u)) & 1023u);   // SWIZZLE_128B tiles need 1024-byte alignment
+  float* epi_tiles = reinterpret_cast<float*>(smem + (size_t)F_S * F_STAGE_BYTES);
+  const int64_t M = *a.Mptr * a.m_mul;
+  const int64_t n_mt = (M + F_M - 1) / F_M;
+  const int64_t n_tiles = n_mt * fa.n_nt;
+  const int nk = fa.nk;
+
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "r"(512));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  if (tid == 32) {
+    for (int s = 0; s < F_S; ++s) {
+      mbar_init(&raw_full[s], 1); mbar_init(&raw_empty[s], F_CVT); mbar_init(&cvt_full[s], F_CVT);
+      mbar_init(&b_full[s], 1); mbar_init(&mma_done[s], 1);
+    }
+    mbar_init(&acc_full, 1); mbar_init(&acc_empty, F_EPI);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t tmem_d0 = tmem_base_s, tmem_d1 = tmem_base_s + F_NT;
+
+  if (warp < 2) {
+    // ---- A producer: TMA loads of the raw fp32 stages, the two warps take alternate stages
+    if (lane == 0) {
+      uint32_t it = 0;
+      for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const int mt = (int)(tile / fa.n_nt);
+        for (int ks = 0; ks < nk; ++ks, ++it) {
+          if ((int)(it & 1) != warp) continue;
+          const uint32_t slot = it % F_S, ph = (it / F_S) & 1;
+          mbar_wait_b(&raw_empty[slot], ph ^ 1);
+          asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&raw_full[slot])), "r"(F_RAW_BYTES) : "memory");
+          uint8_t* dst = smem + (size_t)slot * F_STAGE_BYTES;
+          if (ks < fa.nk0) tma_load_2d(dst, &tmA0, ks * F_KS, mt * F_M, &raw_full[slot]);
+          else tma_load_2d(dst, &tmA1, (ks - fa.nk0) * F_KS, mt * F_M, &raw_full[slot]);
+        }
+      }
+    }
+  } else if (warp < 4) {
+    // ---- B producer: one bulk copy per stage (hi | lo block of this column tile)
+    if (lane == 0) {
+      const int w = warp - 2;
+      uint32_t it = 0;
+      for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const int nt = (int)(tile % fa.n_nt);
+        const int Nt = min(fa.Npad - nt * F_NT, F_NT);
+        const uint8_t* tb = fa.Bp + (size_t)nt * F_NT * fa.Kpad * 4;
+        for (int ks = 0; ks < nk; ++ks, ++it) {
+          if ((int)(it & 1) != w) continue;
+          const uint32_t slot = it % F_S, ph = (it / F_S) & 1;
+          mbar_wait_b(&mma_done[slot], ph ^ 1);
+          bulk_g2s(smem + (size_t)slot * F_STAGE_BYTES + F_OFF_B, tb + (size_t)ks * Nt * (F_KS * 4), (uint32_t)Nt * (F_KS * 4), &b_full[slot]);
+        }
+      }
+    }
+  } else if (warp == F_W_MMA) {
+    // ---- MMA issuer
+    if (lane == 0) {
+      uint32_t it = 0, titer = 0;
+      for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++titer) {
+        const int nt = (int)(tile % fa.n_nt);
+        const int Nt = min(fa.Npad - nt * F_NT, F_NT);
+        // D fp32 (bit 4), A/B fp16 (0 at bits 7 and 10), both K-major, N >> 3 at bit 17, M >> 4 at bit 24
+        const uint32_t idesc = (1u << 4) | ((uint32_t)(Nt >> 3) << 17) | ((uint32_t)(F_M >> 4) << 24);
+        mbar_wait_b(&acc_empty, (titer & 1) ^ 1);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        for (int ks = 0; ks < nk; ++ks, ++it) {
+          const uint32_t slot = it % F_S, ph = (it / F_S) & 1;
+          mbar_wait_b(&cvt_full[slot], ph);
+          mbar_wait_b(&b_full[slot], ph);
+          asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+          const uint32_t sbase = smem_u32(smem + (size_t)slot * F_STAGE_BYTES);
+          const uint32_t sa_hi = sbase + F_OFF_CVT, sa_lo = sa_hi + F_CVT_BYTES;
+          const uint32_t sb_hi = sbase + F_OFF_B, sb_lo = sb_hi + (uint32_t)Nt * (F_KS * 2);
+#pragma unroll
+          for (int k2 = 0; k2 < F_KS / 16; ++k2) {
+            const uint32_t koff = k2 * 256;                     // two 128-byte core-matrix columns per K = 16 step
+            const uint64_t dAh = umma_desc(sa_hi + koff, 128, 512), dAl = umma_desc(sa_lo + koff, 128, 512);
+            const uint64_t dBh = umma_desc(sb_hi + koff, 128, 512), dBl = umma_desc(sb_lo + koff, 128, 512);
+            const uint32_t acc = (ks > 0 || k2 > 0) ? 1u : 0u;
+            umma_f16(tmem_d0, dAh, dBh, idesc, acc);
+            if (fa.passes >= 3) umma_f16(tmem_d1, dAh, dBl, idesc, acc);
+            if (fa.passes >= 2) umma_f16(tmem_d1, dAl, dBh, idesc, fa.passes >= 3 ? 1u : acc);
+          }
+          umma_commit(&mma_done[slot]);
+        }
+        umma_commit(&acc_full);
+      }
+    }
+  } else if (warp < F_W_EPI0) {
+    // ---- converters: raw fp32 stage -> prologue -> hi / lo fp16 canonical tiles.  Lane l of a warp: rows 16 cw + 8 i + (l & 7)
+    // (i = 0, 1), k chunk q = l >> 3 (8 elements): a quarter-warp reads 8 rows of one chunk pair (8 distinct swizzled positions)
+    // and writes 128 contiguous bytes.
+    const int cw = warp - F_W_CVT0;
+    const int q = lane >> 3, r7 = lane & 7;
+    uint32_t it = 0;
+    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+      const int64_t row0 = (tile / fa.n_nt) * F_M;
+      float sc[2] = {1.f, 1.f};
+      if (a.pro == PRO_SCALE_U) {
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+          const int64_t row = row0 + 16 * cw + 8 * i + r7;
+          sc[i] = row < M ? a.c_new * a.geo[row * GEO_W + 4] : 0.f;
+        }
+      }
+      for (int ks = 0; ks < nk; ++ks, ++it) {
+        const uint32_t slot = it % F_S, ph = (it / F_S) & 1;
+        uint8_t* st = smem + (size_t)slot * F_STAGE_BYTES;
+        mbar_wait_b(&raw_full[slot], ph);
+        mbar_wait_b(&mma_done[slot], ph ^ 1);
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+          const int r = 16 * cw + 8 * i + r7;
+          const uint8_t* rp = st + r * 128;
+          const float4 v0 = *reinterpret_cast<const float4*>(rp + (((2 * q) ^ r7) << 4));
+          const float4 v1 = *reinterpret_cast<const float4*>(rp + (((2 * q + 1) ^ r7) << 4));
+          float v[8] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
+          if (a.pro == PRO_SILU) {
+#pragma unroll
+            for (int e = 0; e < 8; ++e) v[e] = silu_f(v[e]);
+          } else if (a.pro == PRO_SCALE_U) {
+#pragma unroll
+            for (int e = 0; e < 8; ++e) v[e] *= sc[i];
+          }
+          uint4 hi, lo;
+          split8(v, hi, lo);
+          const uint32_t off = (uint32_t)(r >> 3) * 512 + q * 128 + r7 * 16;
+          *reinterpret_cast<uint4*>(st + F_OFF_CVT + off) = hi;
+          *reinterpret_cast<uint4*>(st + F_OFF_CVT + F_CVT_BYTES + off) = lo;
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy stores -> visible to the tensor core
+        __syncwarp();
+        if (lane == 0) { mbar_arrive(&cvt_full[slot]); mbar_arrive(&raw_empty[slot]); }
+      }
+    }
+  } else {
+    // ---- epilogue: TMEM lane quadrant = warp % 4; the two warps of a quadrant take alternate 16-column steps
+    const int ew = warp - F_W_EPI0;
+    const int quad = warp & 3, half = ew >> 2;
+    const int erow = quad * 32 + lane;
+    const uint32_t lane_addr = (uint32_t)(quad * 32) << 16;
+    float* wtile = epi_tiles + (size_t)ew * 2 * F_TILE_FLOATS;
+    float* xtile = wtile + F_TILE_FLOATS;
+    const bool mapped = a.cmap_d3 != 0;
+    uint32_t titer = 0;
+    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++titer) {
+      const int mt = (int)(tile / fa.n_nt), nt = (int)(tile % fa.n_nt);
+      const int col0 = nt * F_NT, Nt = min(fa.Npad - col0, F_NT);
+      const int64_t row0 = (int64_t)mt * F_M, row = row0 + erow, rbase = row0 + quad * 32;
+      const bool row_ok = row < M;
+      float u = 0.f; int zi = 0, zj = 0;
+      if (row_ok && a.geo && a.m_mul == 1) {
+        const float* gq = a.geo + row * GEO_W;
+        u = gq[4]; zi = __float_as_int(gq[6]); zj = __float_as_int(gq[7]);
+      }
+      const float* xsrc = (a.epi == EPI_ACCUM) ? a.C : a.aux;
+      const int ldx = (a.epi == EPI_ACCUM) ? a.ldc : a.ldaux;
+      mbar_wait_b(&acc_full, titer & 1);
+      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll 1
+      for (int n0 = half * 16; n0 < Nt; n0 += 32) {
+        const int nb = col0 + n0;                                 // first global column of this step
+        const bool need_x = a.epi == EPI_RESIDUAL || a.epi == EPI_DSILU || a.epi == EPI_ACCUM || (a.epi == EPI_SPLIT_RES && nb < a.split);
+        float4 x[4];
+        if (need_x) {
+          float4 t[4];
+          warp_tile_ldg(t, lane, xsrc, ldx, rbase, M, nb, a.epi == EPI_SPLIT_RES ? a.split : a.N);
+          warp_tile_xpose(xtile, t, x, lane);
+        }
+        float v[16];
+        tmem_ld16(tmem_d0 + lane_addr + (uint32_t)n0, v);
+        if (fa.passes >= 2) {
+          float w[16];
+          tmem_ld16(tmem_d1 + lane_addr + (uint32_t)n0, w);
+#pragma unroll
+          for (int j = 0; j < 16; ++j) v[j] = fmaf(w[j], F_LO_INV, v[j]);
+        }
+        float4 o1[4], o2[4];
+#define F_V(j) make_float4(v[4 * (j)], v[4 * (j) + 1], v[4 * (j) + 2], v[4 * (j) + 3])
+        switch (a.epi) {
+          case EPI_GATHER2: {
+            const float* g1p = fa.WgT + (int64_t)zi * a.N;
+            const float* g2p = fa.WgT + (int64_t)(a.S + zj) * a.N;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              const int nn = min(nb + 4 * j, a.N - 4);            // padded columns read a valid address; they are masked by the store
+              const float4 g1 = *reinterpret_cast<const float4*>(g1p + nn);
+              const float4 g2 = *reinterpret_cast<const float4*>(g2p + nn);
+              const float4 t = F_V(j);
+              o1[j] = make_float4(t.x + (g1.x + g2.x), t.y + (g1.y + g2.y), t.z + (g1.z + g2.z), t.w + (g1.w + g2.w));
+            }
+          } break;
+          case EPI_Y_X:
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              const float4 t = F_V(j);
+              o1[j] = t; o2[j] = make_float4(u * t.x, u * t.y, u * t.z, u * t.w);
+            }
+            break;
+          case EPI_RESIDUAL: {
+            const float cu = a.c_new * u;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              const float4 t = F_V(j);
+              o1[j] = t;
+              o2[j] = make_float4(a.c_old * x[j].x + cu * t.x, a.c_old * x[j].y + cu * t.y, a.c_old * x[j].z + cu * t.z, a.c_old * x[j].w + cu * t.w);
+            }
+          } break;
+          case EPI_DSILU:
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              const float4 t = F_V(j);
+              o1[j] = make_float4(t.x * dsilu_f(x[j].x), t.y * dsilu_f(x[j].y), t.z * dsilu_f(x[j].z), t.w * dsilu_f(x[j].w));
+            }
+            break;
+          case EPI_ACCUM:
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              const float4 t = F_V(j);
+              o1[j] = make_float4(x[j].x + t.x, x[j].y + t.y, x[j].z + t.z, x[j].w + t.w);
+            }
+            break;
+          case EPI_SPLIT_RES: {
+            const bool res = nb < a.split;                        // split % 16 == 0: a step lies on one side
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              const float4 t = F_V(j);
+              o1[j] = res ? make_float4(a.c_old * x[j].x + t.x, a.c_old * x[j].y + t.y, a.c_old * x[j].z + t.z, a.c_old * x[j].w + t.w) : t;
+            }
+          } break;
+          default:
+#pragma unroll
+            for (int j = 0; j < 4; ++j) o1[j] = F_V(j);
+            break;
+        }
+#undef F_V
+        if (a.epi == EPI_SPLIT_RES && nb >= a.split) {
+          tile_store_map(wtile, o1, lane, a, a.C2, a.ldc2, rbase, M, nb - a.split, a.N - a.split, false);
+        } else {
+          tile_store_map(wtile, o1, lane, a, a.C, a.ldc, rbase, M, nb, a.epi == EPI_SPLIT_RES ? a.split : a.N, mapped);
+          if (a.epi == EPI_Y_X || a.epi == EPI_RESIDUAL) tile_store_map(wtile, o2, lane, a, a.C2, a.ldc2, rbase, M, nb, a.N, false);
+        }
+      }
+      asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&acc_empty);
+    }
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (warp == 0) {
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_d0), "r"(512));
+  }
+}
+
+// ---- host side -------------------------------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess) p = nullptr;
+    cudaGetLastError();
+    return reinterpret_cast<EncodeTiledFn>(p);
+  }();
+  return fn;
+}
+
+// fp32 matrix [rows][K] with leading dimension ld, boxes of 32 columns x 128 rows, SWIZZLE_128B, zero fill outside
+bool make_map(Model* m, const float* A, int K, int ld, int64_t rows, CUtensorMap* out) {
+  const std::array<int64_t, 4> key = {(int64_t)(uintptr_t)A, K, ld, rows};
+  auto it = m->tmaps.find(key);
+  if (it != m->tmaps.end()) { std::memcpy(out, &it->second, sizeof(CUtensorMap)); return true; }
+  EncodeTiledFn enc = encode_fn();
+  if (!enc) return false;
+  cuuint64_t gdim[2] = {(cuuint64_t)K, (cuuint64_t)rows};
+  cuuint64_t gstr[1] = {(cuuint64_t)ld * 4};
+  cuuint32_t box[2] = {(cuuint32_t)F_KS, (cuuint32_t)F_M};
+  cuuint32_t estr[2] = {1, 1};
+  CUtensorMap tm;
+  if (enc(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(A), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+          CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+    return false;
+  TMapStore s;
+  static_assert(sizeof(TMapStore) == sizeof(CUtensorMap), "tensor map storage");
+  std::memcpy(&s, &tm, sizeof(tm));
+  if (m->tmaps.size() > 4096) m->tmaps.clear();   // workspace reallocations leave dead entries behind
+  m->tmaps[key] = s;
+  std::memcpy(out, &tm, sizeof(tm));
+  return true;
+}
+
+uint8_t* packed_weights16(Model* m, const GemmArgs& a, cudaStream_t st, int* Npad_out, int* Kpad_out) {
+  const int K = a.K0 + a.K1;
+  const int Npad = (a.N + 15) / 16 * 16, Kpad = (K + F_KS - 1) / F_KS * F_KS;
+  *Npad_out = Npad; *Kpad_out = Kpad;
+  const std::array<int64_t, 5> key = {(int64_t)(a.W - m->d_w), a.ldw, a.wtrans | 16, a.N, K};
+  auto it = m->packed_w.find(key);
+  if (it != m->packed_w.end()) return reinterpret_cast<uint8_t*>(it->second);
+  float* Bp = nullptr;
+  if (cudaMalloc(&Bp, 4 * (size_t)Npad * Kpad) != cudaSuccess) { cudaGetLastError(); m->err = "packed weight allocation failed"; return nullptr; }
+  const int64_t tot = (int64_t)Npad * Kpad;
+  k_pack_w16<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(a.W, a.ldw, a.wtrans, a.N, K, Npad, Kpad, reinterpret_cast<uint8_t*>(Bp));
+  m->packed_w[key] = Bp;
+  return reinterpret_cast<uint8_t*>(Bp);
+}
+
+}  // namespace
+
+// Returns false when the shape / alignment is outside what the kernel takes (the caller then uses k_gemm_tc).
+bool launch_gemm_f16s(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st) {
+  const int K = a.K0 + a.K1;
+  auto al = [](const void* p) { return ((uintptr_t)p & 15) == 0; };
+  if (a.amap_d3) return false;                                                    // mapped A rows: not a 2-D tensor map
+  if (K < 1 || a.N < 4 || a.N % 4 || a.lda0 % 4 || !al(a.A0)) return false;
+  if (a.K1 > 0 && (a.K0 % F_KS || a.lda1 % 4 || !al(a.A1))) return false;
+  if (a.ldc % 4 || !al(a.C)) return false;
+  if (a.C2 && (a.ldc2 % 4 || !al(a.C2))) return false;
+  if (a.aux && (a.ldaux % 4 || !al(a.aux))) return false;
+  if (a.epi == EPI_SPLIT_RES && a.split % 16) return false;
+  if (a.m_mul != 1 && (a.epi != EPI_STORE || a.pro != PRO_NONE)) return false;
+  if (m->f16_rows_cap <= 0) return false;
+  FArgs fa{};
+  fa.a = a;
+  fa.passes = m->f16_passes;
+  uint8_t* Bp = packed_weights16(m, a, st, &fa.Npad, &fa.Kpad);
+  if (!Bp) return false;
+  fa.Bp = Bp;
+  fa.n_nt = (fa.Npad + F_NT - 1) / F_NT;
+  fa.nk0 = (a.K0 + F_KS - 1) / F_KS;
+  fa.nk = fa.nk0 + (a.K1 + F_KS - 1) / F_KS;
+  fa.WgT = nullptr;
+  if (a.epi == EPI_GATHER2) {
+    fa.WgT = transposed_species_columns(m, a, st);
+    if (!fa.WgT) return false;
+  }
+  const int64_t rows_cap = m->f16_rows_cap * a.m_mul;                              // rows the A buffers hold (workspace capacity)
+  CUtensorMap t0, t1;
+  if (!make_map(m, a.A0, a.K0, a.lda0, rows_cap, &t0)) return false;
+  if (a.K1 > 0) { if (!make_map(m, a.A1, a.K1, a.lda1, rows_cap, &t1)) return false; }
+  else t1 = t0;
+  static int attr_dev = -1;
+  if (attr_dev != m->device) {
+    if (cudaFuncSetAttribute(k_gemm_f16s, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F_SMEM) != cudaSuccess) { cudaGetLastError(); return false; }
+    attr_dev = m->device;
+  }
+  const int64_t tiles = ((m_cap * a.m_mul + F_M - 1) / F_M) * fa.n_nt;
+  const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(tiles, m->num_sms));
+  prof_begin(m, st, KC_GEMM, 2.0 * a.N * K * a.m_mul);
+  k_gemm_f16s<<<grid, F_T, F_SMEM, st>>>(fa, t0, t1);
+  prof_end(m, st);
+  m->launches += 1;
+  return true;
+}
+
+}  // namespace allegro

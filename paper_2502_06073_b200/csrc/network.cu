@@ -111,6 +111,7 @@ int ws_prepare(Model* m, int64_t cap_edges, int64_t cap_atoms) {
   ws.Tbig = m->use_big ? cf(E * tbig_per_edge(P)) : nullptr;
   if (off > total) { m->err = "internal: workspace carve overflow"; return ALLEGRO_ERR_ALLOC; }
   ws.cap_edges = cap_edges; ws.cap_atoms = cap_atoms;
+  m->f16_rows_cap = cap_edges;
   return 0;
 }
 
