@@ -1,5 +1,6 @@
 // api.cu — the C-ABI entry points declared in include/allegro.h (argument checking, ownership, error codes).
 #include <cmath>
+#include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <new>

@@ -19,8 +19,14 @@
 //     the per-row c_new u scale), split hi / lo and write the canonical K-major UMMA tiles;
 //   * 1 thread issues the 2 x 3 tcgen05.mma.kind::f16 (M = 128, N <= 256, K = 16) of a stage and commits them to the stage
 //     barrier, which frees the converted A tile and the weight slot;
-//   * 8 epilogue warps (two per TMEM lane quadrant) read D0 / D1 with tcgen05.ld, combine, apply the fused epilogue and move
-//     rows through per-warp swizzled tiles so that every global access covers full 32-byte sectors.
+//   * 8 epilogue warps (two groups of four, one warp per TMEM lane quadrant) read D0 / D1 with tcgen05.ld, combine, apply the
+//     fused epilogue, write a 128 x 32 output tile into shared memory (SWIZZLE_128B, conflict-free one row per lane) and one
+//     thread hands it to the TMA unit (cp.async.bulk.tensor store): address generation, coalescing and clipping at the
+//     matrix edge cost no instructions (the per-warp transposition tiles of gemm_tc.cu cost ~530 SASS instructions per 16
+//     columns, profiles/r2_c_f16s.md).  Rows between the number of active edges and the end of the last tile are written
+//     with don't-care values: every edge-sized workspace array holds the full capacity.
+//   * rows may be (edge, m) pairs of one irrep inside an [e][comp][c] tensor (tp_big.cuh): tiles then hold d3 * floor(128 / d3)
+//     rows and the mapped operand is a 3-D tensor map (c, m, e).
 // D0 + D1 take all 512 TMEM columns for a 256-column tile, so the accumulators are single-buffered: the loads and the
 // conversions of the next tile run during the epilogue, the tensor pipe waits for it.
 #include <cuda.h>
@@ -46,8 +52,8 @@ constexpr uint32_t F_CVT_BYTES = F_M * F_KS * 2;                        // one o
 constexpr uint32_t F_BMAX_BYTES = F_NT * F_KS * 2;                      // one of B_hi / B_lo at 256 columns
 constexpr uint32_t F_OFF_CVT = F_RAW_BYTES, F_OFF_B = F_RAW_BYTES + 2 * F_CVT_BYTES;
 constexpr uint32_t F_STAGE_BYTES = F_OFF_B + 2 * F_BMAX_BYTES;          // 64 KB
-constexpr uint32_t F_TILE_FLOATS = 32 * WT_LD;                          // per-warp transposition tile
-constexpr size_t F_SMEM = (size_t)F_S * F_STAGE_BYTES + (size_t)F_EPI * 2 * F_TILE_FLOATS * 4 + 1024;
+constexpr uint32_t F_OUT_BYTES = F_M * 32 * 4;                          // one 128 x 32 fp32 output tile per epilogue group
+constexpr size_t F_SMEM = (size_t)F_S * F_STAGE_BYTES + 2 * F_OUT_BYTES + 1024;
 constexpr float F_LO_SCALE = 2048.0f, F_LO_INV = 1.0f / 2048.0f;
 
 struct FArgs {
@@ -57,10 +63,12 @@ struct FArgs {
   int Npad, Kpad, n_nt;     // N padded to 16, K to 32, number of column tiles
   int nk0, nk;              // K stages that read A0, total
   int passes;               // 3 = full split, 2 = activations split only, 1 = plain fp16 (precision study)
+  int rpt;                  // rows per tile: 128, or d3 * (128 / d3) when rows are (edge, m) pairs of a mapped operand
+  int a_d3, c_d3;           // > 0: A0 / C is the 3-D mapped tensor
 };
 
+// bounded wait: a protocol error ends in a trap (sticky CUDA error) instead of a hung GPU
 __device__ __forceinline__ void mbar_wait_b(uint64_t* bar, uint32_t parity) {
-  // bounded: a protocol error ends in a trap (sticky CUDA error) instead of a hung GPU
   uint32_t done = 0;
   for (uint32_t it = 0; !done; ++it) {
     asm volatile(
@@ -79,6 +87,18 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
 __device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* tm, int c0, int c1, uint64_t* bar) {
   asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(smem_u32(dst)),
                "l"(tm), "r"(c0), "r"(c1), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, int c0, int c1, int c2, uint64_t* bar) {
+  asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(smem_u32(dst)),
+               "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* tm, int c0, int c1, const void* src) {
+  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];" ::"l"(tm), "r"(c0), "r"(c1), "r"(smem_u32(src)) : "memory");
+}
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* tm, int c0, int c1, int c2, const void* src) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(src))
                : "memory");
 }
 __device__ __forceinline__ void umma_f16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
@@ -120,30 +140,9 @@ __global__ void k_pack_w16(const float* __restrict__ W, int ldw, int wtrans, int
   *reinterpret_cast<__half*>(out + base + (size_t)Nt * (F_KS * 2) + off) = lo;
 }
 
-// row r of the GEMM -> row of the C tensor (tp_big.cuh: (edge, m) pairs of one irrep inside [e][comp][c])
-__device__ __forceinline__ int64_t crow(const GemmArgs& a, int64_t r) {
-  return a.cmap_d3 ? (r / a.cmap_d3) * a.cmap_od + a.cmap_off + r % a.cmap_d3 : r;
-}
-// per-warp tile store of 32 rows x 16 columns with the row map applied
-__device__ __forceinline__ void tile_store_map(float* tile, const float4 (&o)[4], int lane, const GemmArgs& a, float* C, int ld, int64_t rbase,
-                                               int64_t M, int col0, int N, bool mapped) {
-#pragma unroll
-  for (int j = 0; j < 4; ++j) *reinterpret_cast<float4*>(tile + wt_off(lane, j)) = o[j];
-  __syncwarp();
-  const int cq = (lane & 3) * 4;
-  float4 t[4];
-#pragma unroll
-  for (int i = 0; i < 4; ++i) t[i] = *reinterpret_cast<const float4*>(tile + wt_off(i * 8 + (lane >> 2), lane & 3));
-#pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const int64_t r = rbase + i * 8 + (lane >> 2);
-    if (r < M && col0 + cq < N) *reinterpret_cast<float4*>(C + (mapped ? crow(a, r) : r) * ld + col0 + cq) = t[i];
-  }
-  __syncwarp();
-}
-
 __global__ void __launch_bounds__(F_T, 1) k_gemm_f16s(const __grid_constant__ FArgs fa, const __grid_constant__ CUtensorMap tmA0,
-                                                       const __grid_constant__ CUtensorMap tmA1) {
+                                                       const __grid_constant__ CUtensorMap tmA1, const __grid_constant__ CUtensorMap tmC,
+                                                       const __grid_constant__ CUtensorMap tmC2) {
   extern __shared__ uint8_t smem_dyn[];
   __shared__ __align__(8) uint64_t raw_full[F_S], raw_empty[F_S], cvt_full[F_S], b_full[F_S], mma_done[F_S];
   __shared__ __align__(8) uint64_t acc_full, acc_empty;
@@ -151,11 +150,13 @@ __global__ void __launch_bounds__(F_T, 1) k_gemm_f16s(const __grid_constant__ FA
   const GemmArgs& a = fa.a;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   uint8_t* smem = smem_dyn + ((1024u - (smem_u32(smem_dyn) & 1023u)) & 1023u);   // SWIZZLE_128B tiles need 1024-byte alignment
-  float* epi_tiles = reinterpret_cast<float*>(smem + (size_t)F_S * F_STAGE_BYTES);
+  uint8_t* out_tiles = smem + (size_t)F_S * F_STAGE_BYTES;
   const int64_t M = *a.Mptr * a.m_mul;
-  const int64_t n_mt = (M + F_M - 1) / F_M;
+  const int rpt = fa.rpt;
+  const int64_t n_mt = (M + rpt - 1) / rpt;
   const int64_t n_tiles = n_mt * fa.n_nt;
   const int nk = fa.nk;
+  const int passes = fa.passes;
 
   if (warp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&tmem_base_s)), "r"(512));
@@ -177,6 +178,8 @@ __global__ void __launch_bounds__(F_T, 1) k_gemm_f16s(const __grid_constant__ FA
   if (warp < 2) {
     // ---- A producer: TMA loads of the raw fp32 stages, the two warps take alternate stages
     if (lane == 0) {
+      const uint32_t a0_bytes = fa.a_d3 ? (uint32_t)rpt * (F_KS * 4) : F_RAW_BYTES;
+      const int epb = fa.a_d3 ? rpt / fa.a_d3 : 0;                      // edges per tile of the mapped operand
       uint32_t it = 0;
       for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const int mt = (int)(tile / fa.n_nt);
@@ -184,10 +187,15 @@ __global__ void __launch_bounds__(F_T, 1) k_gemm_f16s(const __grid_constant__ FA
           if ((int)(it & 1) != warp) continue;
           const uint32_t slot = it % F_S, ph = (it / F_S) & 1;
           mbar_wait_b(&raw_empty[slot], ph ^ 1);
-          asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&raw_full[slot])), "r"(F_RAW_BYTES) : "memory");
           uint8_t* dst = smem + (size_t)slot * F_STAGE_BYTES;
-          if (ks < fa.nk0) tma_load_2d(dst, &tmA0, ks * F_KS, mt * F_M, &raw_full[slot]);
-          else tma_load_2d(dst, &tmA1, (ks - fa.nk0) * F_KS, mt * F_M, &raw_full[slot]);
+          if (ks < fa.nk0) {
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&raw_full[slot])), "r"(a0_bytes) : "memory");
+            if (fa.a_d3) tma_load_3d(dst, &tmA0, ks * F_KS, 0, mt * epb, &raw_full[slot]);
+            else tma_load_2d(dst, &tmA0, ks * F_KS, mt * rpt, &raw_full[slot]);
+          } else {
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&raw_full[slot])), "r"(F_RAW_BYTES) : "memory");
+            tma_load_2d(dst, &tmA1, (ks - fa.nk0) * F_KS, mt * rpt, &raw_full[slot]);
+          }
         }
       }
     }
@@ -234,8 +242,8 @@ __global__ void __launch_bounds__(F_T, 1) k_gemm_f16s(const __grid_constant__ FA
             const uint64_t dBh = umma_desc(sb_hi + koff, 128, 512), dBl = umma_desc(sb_lo + koff, 128, 512);
             const uint32_t acc = (ks > 0 || k2 > 0) ? 1u : 0u;
             umma_f16(tmem_d0, dAh, dBh, idesc, acc);
-            if (fa.passes >= 3) umma_f16(tmem_d1, dAh, dBl, idesc, acc);
-            if (fa.passes >= 2) umma_f16(tmem_d1, dAl, dBh, idesc, fa.passes >= 3 ? 1u : acc);
+            if (passes >= 3) umma_f16(tmem_d1, dAh, dBl, idesc, acc);
+            if (passes >= 2) umma_f16(tmem_d1, dAl, dBh, idesc, passes >= 3 ? 1u : acc);
           }
           umma_commit(&mma_done[slot]);
         }
@@ -250,7 +258,7 @@ __global__ void __launch_bounds__(F_T, 1) k_gemm_f16s(const __grid_constant__ FA
     const int q = lane >> 3, r7 = lane & 7;
     uint32_t it = 0;
     for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-      const int64_t row0 = (tile / fa.n_nt) * F_M;
+      const int64_t row0 = (tile / fa.n_nt) * rpt;
       float sc[2] = {1.f, 1.f};
       if (a.pro == PRO_SCALE_U) {
 #pragma unroll
@@ -290,117 +298,141 @@ __global__ void __launch_bounds__(F_T, 1) k_gemm_f16s(const __grid_constant__ FA
       }
     }
   } else {
-    // ---- epilogue: TMEM lane quadrant = warp % 4; the two warps of a quadrant take alternate 16-column steps
+    // ---- epilogue: two groups of four warps (TMEM lane quadrant = warp % 4); a group takes alternate 32-column steps, builds
+    // the 128 x 32 output tile in shared memory (row per lane, 16-byte chunks XOR-swizzled like the tensor map) and TMA-stores it.
     const int ew = warp - F_W_EPI0;
-    const int quad = warp & 3, half = ew >> 2;
+    const int quad = warp & 3, grp = ew >> 2;
     const int erow = quad * 32 + lane;
     const uint32_t lane_addr = (uint32_t)(quad * 32) << 16;
-    float* wtile = epi_tiles + (size_t)ew * 2 * F_TILE_FLOATS;
-    float* xtile = wtile + F_TILE_FLOATS;
-    const bool mapped = a.cmap_d3 != 0;
+    uint8_t* obuf = out_tiles + (size_t)grp * F_OUT_BYTES;
+    uint8_t* orow = obuf + erow * 128;
+    const int sw = erow & 7;
+    const bool leader = (quad == 0 && lane == 0);            // issues the stores of its group
+    const int bar_id = 1 + grp;
+    const int epb_c = fa.c_d3 ? rpt / fa.c_d3 : 0;
+    const int npass = (a.epi == EPI_Y_X || a.epi == EPI_RESIDUAL) ? 2 : 1;
     uint32_t titer = 0;
     for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++titer) {
       const int mt = (int)(tile / fa.n_nt), nt = (int)(tile % fa.n_nt);
       const int col0 = nt * F_NT, Nt = min(fa.Npad - col0, F_NT);
-      const int64_t row0 = (int64_t)mt * F_M, row = row0 + erow, rbase = row0 + quad * 32;
-      const bool row_ok = row < M;
+      const int64_t row0 = (int64_t)mt * rpt, row = row0 + erow;
+      const bool row_ok = row < M && erow < rpt;
       float u = 0.f; int zi = 0, zj = 0;
       if (row_ok && a.geo && a.m_mul == 1) {
         const float* gq = a.geo + row * GEO_W;
         u = gq[4]; zi = __float_as_int(gq[6]); zj = __float_as_int(gq[7]);
       }
-      const float* xsrc = (a.epi == EPI_ACCUM) ? a.C : a.aux;
-      const int ldx = (a.epi == EPI_ACCUM) ? a.ldc : a.ldaux;
+      const float* xrow = ((a.epi == EPI_ACCUM) ? a.C + row * a.ldc : a.aux + row * a.ldaux);
+      const float cu = a.c_new * u;
       mbar_wait_b(&acc_full, titer & 1);
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll 1
-      for (int n0 = half * 16; n0 < Nt; n0 += 32) {
-        const int nb = col0 + n0;                                 // first global column of this step
-        const bool need_x = a.epi == EPI_RESIDUAL || a.epi == EPI_DSILU || a.epi == EPI_ACCUM || (a.epi == EPI_SPLIT_RES && nb < a.split);
-        float4 x[4];
-        if (need_x) {
-          float4 t[4];
-          warp_tile_ldg(t, lane, xsrc, ldx, rbase, M, nb, a.epi == EPI_SPLIT_RES ? a.split : a.N);
-          warp_tile_xpose(xtile, t, x, lane);
-        }
-        float v[16];
-        tmem_ld16(tmem_d0 + lane_addr + (uint32_t)n0, v);
-        if (fa.passes >= 2) {
-          float w[16];
-          tmem_ld16(tmem_d1 + lane_addr + (uint32_t)n0, w);
+      for (int c32 = grp; c32 * 32 < Nt; c32 += 2) {
+        const int nb = col0 + c32 * 32;                          // first global column of this step
+        const bool to_c2 = a.epi == EPI_SPLIT_RES && nb >= a.split;
+        const int xlim = a.epi == EPI_SPLIT_RES ? a.split : a.N;
+        const bool need_x = a.epi == EPI_DSILU || a.epi == EPI_ACCUM || (a.epi == EPI_SPLIT_RES && !to_c2);
+#pragma unroll 1
+        for (int pass = 0; pass < npass; ++pass) {
+          // the previous store of this group has finished reading the tile
+          if (leader) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+          asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
 #pragma unroll
-          for (int j = 0; j < 16; ++j) v[j] = fmaf(w[j], F_LO_INV, v[j]);
-        }
-        float4 o1[4], o2[4];
+          for (int sub = 0; sub < 2; ++sub) {
+            const int n0 = c32 * 32 + sub * 16, ng = col0 + n0;
+            float v[16];
+            tmem_ld16(tmem_d0 + lane_addr + (uint32_t)n0, v);
+            if (passes >= 2) {
+              float w[16];
+              tmem_ld16(tmem_d1 + lane_addr + (uint32_t)n0, w);
+#pragma unroll
+              for (int j = 0; j < 16; ++j) v[j] = fmaf(w[j], F_LO_INV, v[j]);
+            }
+            float4 x[4];
+            const bool ldx = (need_x || (a.epi == EPI_RESIDUAL && pass == 1)) && row_ok;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              x[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+              if (ldx && ng + 4 * j < xlim) x[j] = *reinterpret_cast<const float4*>(xrow + ng + 4 * j);
+            }
+            float4 o[4];
 #define F_V(j) make_float4(v[4 * (j)], v[4 * (j) + 1], v[4 * (j) + 2], v[4 * (j) + 3])
-        switch (a.epi) {
-          case EPI_GATHER2: {
-            const float* g1p = fa.WgT + (int64_t)zi * a.N;
-            const float* g2p = fa.WgT + (int64_t)(a.S + zj) * a.N;
+            switch (a.epi) {
+              case EPI_GATHER2: {
+                const float* g1p = fa.WgT + (int64_t)zi * a.N;
+                const float* g2p = fa.WgT + (int64_t)(a.S + zj) * a.N;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const int nn = min(nb + 4 * j, a.N - 4);            // padded columns read a valid address; they are masked by the store
-              const float4 g1 = *reinterpret_cast<const float4*>(g1p + nn);
-              const float4 g2 = *reinterpret_cast<const float4*>(g2p + nn);
-              const float4 t = F_V(j);
-              o1[j] = make_float4(t.x + (g1.x + g2.x), t.y + (g1.y + g2.y), t.z + (g1.z + g2.z), t.w + (g1.w + g2.w));
+                for (int j = 0; j < 4; ++j) {
+                  const int nn = min(ng + 4 * j, a.N - 4);        // padded columns read a valid address; the store clips them
+                  const float4 g1 = *reinterpret_cast<const float4*>(g1p + nn);
+                  const float4 g2 = *reinterpret_cast<const float4*>(g2p + nn);
+                  const float4 t = F_V(j);
+                  o[j] = make_float4(t.x + (g1.x + g2.x), t.y + (g1.y + g2.y), t.z + (g1.z + g2.z), t.w + (g1.w + g2.w));
+                }
+              } break;
+              case EPI_Y_X:
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                  const float4 t = F_V(j);
+                  o[j] = pass == 0 ? t : make_float4(u * t.x, u * t.y, u * t.z, u * t.w);
+                }
+                break;
+              case EPI_RESIDUAL:
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                  const float4 t = F_V(j);
+                  o[j] = pass == 0 ? t
+                                   : make_float4(a.c_old * x[j].x + cu * t.x, a.c_old * x[j].y + cu * t.y, a.c_old * x[j].z + cu * t.z,
+                                                 a.c_old * x[j].w + cu * t.w);
+                }
+                break;
+              case EPI_DSILU:
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                  const float4 t = F_V(j);
+                  o[j] = make_float4(t.x * dsilu_f(x[j].x), t.y * dsilu_f(x[j].y), t.z * dsilu_f(x[j].z), t.w * dsilu_f(x[j].w));
+                }
+                break;
+              case EPI_ACCUM:
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                  const float4 t = F_V(j);
+                  o[j] = make_float4(x[j].x + t.x, x[j].y + t.y, x[j].z + t.z, x[j].w + t.w);
+                }
+                break;
+              case EPI_SPLIT_RES:
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                  const float4 t = F_V(j);
+                  o[j] = to_c2 ? t : make_float4(a.c_old * x[j].x + t.x, a.c_old * x[j].y + t.y, a.c_old * x[j].z + t.z, a.c_old * x[j].w + t.w);
+                }
+                break;
+              default:
+#pragma unroll
+                for (int j = 0; j < 4; ++j) o[j] = F_V(j);
+                break;
             }
-          } break;
-          case EPI_Y_X:
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const float4 t = F_V(j);
-              o1[j] = t; o2[j] = make_float4(u * t.x, u * t.y, u * t.z, u * t.w);
-            }
-            break;
-          case EPI_RESIDUAL: {
-            const float cu = a.c_new * u;
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const float4 t = F_V(j);
-              o1[j] = t;
-              o2[j] = make_float4(a.c_old * x[j].x + cu * t.x, a.c_old * x[j].y + cu * t.y, a.c_old * x[j].z + cu * t.z, a.c_old * x[j].w + cu * t.w);
-            }
-          } break;
-          case EPI_DSILU:
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const float4 t = F_V(j);
-              o1[j] = make_float4(t.x * dsilu_f(x[j].x), t.y * dsilu_f(x[j].y), t.z * dsilu_f(x[j].z), t.w * dsilu_f(x[j].w));
-            }
-            break;
-          case EPI_ACCUM:
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const float4 t = F_V(j);
-              o1[j] = make_float4(x[j].x + t.x, x[j].y + t.y, x[j].z + t.z, x[j].w + t.w);
-            }
-            break;
-          case EPI_SPLIT_RES: {
-            const bool res = nb < a.split;                        // split % 16 == 0: a step lies on one side
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const float4 t = F_V(j);
-              o1[j] = res ? make_float4(a.c_old * x[j].x + t.x, a.c_old * x[j].y + t.y, a.c_old * x[j].z + t.z, a.c_old * x[j].w + t.w) : t;
-            }
-          } break;
-          default:
-#pragma unroll
-            for (int j = 0; j < 4; ++j) o1[j] = F_V(j);
-            break;
-        }
 #undef F_V
-        if (a.epi == EPI_SPLIT_RES && nb >= a.split) {
-          tile_store_map(wtile, o1, lane, a, a.C2, a.ldc2, rbase, M, nb - a.split, a.N - a.split, false);
-        } else {
-          tile_store_map(wtile, o1, lane, a, a.C, a.ldc, rbase, M, nb, a.epi == EPI_SPLIT_RES ? a.split : a.N, mapped);
-          if (a.epi == EPI_Y_X || a.epi == EPI_RESIDUAL) tile_store_map(wtile, o2, lane, a, a.C2, a.ldc2, rbase, M, nb, a.N, false);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) *reinterpret_cast<float4*>(orow + (((sub * 4 + j) ^ sw) << 4)) = o[j];
+          }
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // tile stores -> visible to the TMA unit
+          asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
+          if (leader) {
+            const bool second = to_c2 || pass == 1;
+            const CUtensorMap* tm = second ? &tmC2 : &tmC;
+            const int cc = to_c2 ? nb - a.split : nb;
+            if (fa.c_d3 && !second) tma_store_3d(tm, cc, 0, mt * epb_c, obuf);
+            else tma_store_2d(tm, cc, (int)row0, obuf);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+          }
         }
       }
       asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
       __syncwarp();
       if (lane == 0) mbar_arrive(&acc_empty);
     }
+    if (leader) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // all stores complete before the CTA retires
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
@@ -425,21 +457,34 @@ EncodeTiledFn encode_fn() {
   return fn;
 }
 
-// fp32 matrix [rows][K] with leading dimension ld, boxes of 32 columns x 128 rows, SWIZZLE_128B, zero fill outside
-bool make_map(Model* m, const float* A, int K, int ld, int64_t rows, CUtensorMap* out) {
-  const std::array<int64_t, 4> key = {(int64_t)(uintptr_t)A, K, ld, rows};
+// fp32 matrix [rows][K] with leading dimension ld, boxes of 32 columns x 128 rows, SWIZZLE_128B, zero fill / clipping outside.
+// d3 > 0: rows are (edge, m) pairs of one irrep of an [e][comp][c] tensor (A points at its first row): 3-D map (c, m, e) with
+// boxes of 32 x d3 x (128 / d3); od = comps per edge.  box_rows < 128 for the plain side of a mapped GEMM: a store must not
+// touch the rows of the next tile.
+bool make_map(Model* m, const float* A, int K, int ld, int64_t rows, int d3, int od, int box_rows, CUtensorMap* out) {
+  const std::array<int64_t, 6> key = {(int64_t)(uintptr_t)A, K, ld, rows, d3 + 16 * box_rows, od};
   auto it = m->tmaps.find(key);
   if (it != m->tmaps.end()) { std::memcpy(out, &it->second, sizeof(CUtensorMap)); return true; }
   EncodeTiledFn enc = encode_fn();
   if (!enc) return false;
-  cuuint64_t gdim[2] = {(cuuint64_t)K, (cuuint64_t)rows};
-  cuuint64_t gstr[1] = {(cuuint64_t)ld * 4};
-  cuuint32_t box[2] = {(cuuint32_t)F_KS, (cuuint32_t)F_M};
-  cuuint32_t estr[2] = {1, 1};
   CUtensorMap tm;
-  if (enc(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(A), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-          CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-    return false;
+  CUresult r;
+  if (d3 > 0) {
+    cuuint64_t gdim[3] = {(cuuint64_t)K, (cuuint64_t)d3, (cuuint64_t)(rows / d3)};
+    cuuint64_t gstr[2] = {(cuuint64_t)ld * 4, (cuuint64_t)od * ld * 4};
+    cuuint32_t box[3] = {(cuuint32_t)F_KS, (cuuint32_t)d3, (cuuint32_t)(F_M / d3)};
+    cuuint32_t estr[3] = {1, 1, 1};
+    r = enc(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(A), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  } else {
+    cuuint64_t gdim[2] = {(cuuint64_t)K, (cuuint64_t)rows};
+    cuuint64_t gstr[1] = {(cuuint64_t)ld * 4};
+    cuuint32_t box[2] = {(cuuint32_t)F_KS, (cuuint32_t)box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    r = enc(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(A), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  }
+  if (r != CUDA_SUCCESS) return false;
   TMapStore s;
   static_assert(sizeof(TMapStore) == sizeof(CUtensorMap), "tensor map storage");
   std::memcpy(&s, &tm, sizeof(tm));
@@ -470,14 +515,15 @@ uint8_t* packed_weights16(Model* m, const GemmArgs& a, cudaStream_t st, int* Npa
 bool launch_gemm_f16s(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st) {
   const int K = a.K0 + a.K1;
   auto al = [](const void* p) { return ((uintptr_t)p & 15) == 0; };
-  if (a.amap_d3) return false;                                                    // mapped A rows: not a 2-D tensor map
   if (K < 1 || a.N < 4 || a.N % 4 || a.lda0 % 4 || !al(a.A0)) return false;
   if (a.K1 > 0 && (a.K0 % F_KS || a.lda1 % 4 || !al(a.A1))) return false;
   if (a.ldc % 4 || !al(a.C)) return false;
   if (a.C2 && (a.ldc2 % 4 || !al(a.C2))) return false;
   if (a.aux && (a.ldaux % 4 || !al(a.aux))) return false;
-  if (a.epi == EPI_SPLIT_RES && a.split % 16) return false;
+  if (a.epi == EPI_SPLIT_RES && a.split % 32) return false;
   if (a.m_mul != 1 && (a.epi != EPI_STORE || a.pro != PRO_NONE)) return false;
+  if ((a.amap_d3 || a.cmap_d3) && (a.K1 > 0 || a.epi != EPI_STORE)) return false;
+  if (a.amap_d3 && a.cmap_d3 && a.amap_d3 != a.cmap_d3) return false;
   if (m->f16_rows_cap <= 0) return false;
   FArgs fa{};
   fa.a = a;
@@ -493,20 +539,29 @@ bool launch_gemm_f16s(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t s
     fa.WgT = transposed_species_columns(m, a, st);
     if (!fa.WgT) return false;
   }
-  const int64_t rows_cap = m->f16_rows_cap * a.m_mul;                              // rows the A buffers hold (workspace capacity)
-  CUtensorMap t0, t1;
-  if (!make_map(m, a.A0, a.K0, a.lda0, rows_cap, &t0)) return false;
-  if (a.K1 > 0) { if (!make_map(m, a.A1, a.K1, a.lda1, rows_cap, &t1)) return false; }
+  const int d3 = a.amap_d3 ? a.amap_d3 : a.cmap_d3;
+  fa.rpt = d3 ? d3 * (F_M / d3) : F_M;
+  fa.a_d3 = a.amap_d3; fa.c_d3 = a.cmap_d3;
+  const int64_t rows_cap = m->f16_rows_cap * a.m_mul;                              // rows the operand buffers hold (workspace capacity)
+  CUtensorMap t0, t1, tc, tc2;
+  if (a.amap_d3) { if (!make_map(m, a.A0 + (int64_t)a.amap_off * a.lda0, a.K0, a.lda0, rows_cap, a.amap_d3, a.amap_od, F_M, &t0)) return false; }
+  else if (!make_map(m, a.A0, a.K0, a.lda0, rows_cap, 0, 0, F_M, &t0)) return false;
+  if (a.K1 > 0) { if (!make_map(m, a.A1, a.K1, a.lda1, rows_cap, 0, 0, F_M, &t1)) return false; }
   else t1 = t0;
+  const int cw = a.epi == EPI_SPLIT_RES ? a.split : a.N;
+  if (a.cmap_d3) { if (!make_map(m, a.C + (int64_t)a.cmap_off * a.ldc, cw, a.ldc, rows_cap, a.cmap_d3, a.cmap_od, F_M, &tc)) return false; }
+  else if (!make_map(m, a.C, cw, a.ldc, rows_cap, 0, 0, fa.rpt, &tc)) return false;
+  if (a.C2) { if (!make_map(m, a.C2, a.epi == EPI_SPLIT_RES ? a.N - a.split : a.N, a.ldc2, rows_cap, 0, 0, fa.rpt, &tc2)) return false; }
+  else tc2 = tc;
   static int attr_dev = -1;
   if (attr_dev != m->device) {
     if (cudaFuncSetAttribute(k_gemm_f16s, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F_SMEM) != cudaSuccess) { cudaGetLastError(); return false; }
     attr_dev = m->device;
   }
-  const int64_t tiles = ((m_cap * a.m_mul + F_M - 1) / F_M) * fa.n_nt;
+  const int64_t tiles = ((m_cap * a.m_mul + fa.rpt - 1) / fa.rpt) * fa.n_nt;
   const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(tiles, m->num_sms));
   prof_begin(m, st, KC_GEMM, 2.0 * a.N * K * a.m_mul);
-  k_gemm_f16s<<<grid, F_T, F_SMEM, st>>>(fa, t0, t1);
+  k_gemm_f16s<<<grid, F_T, F_SMEM, st>>>(fa, t0, t1, tc, tc2);
   prof_end(m, st);
   m->launches += 1;
   return true;
