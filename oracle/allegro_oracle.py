@@ -585,12 +585,15 @@ class AllegroOracle:
         return E_i, has, g_e
 
     # ------------------------------------------------------------------------------------------
-    def energy_forces(self, pos, species, cell, nbr, centres=None, max_edges_per_chunk=200_000, taps=None):
+    def energy_forces(self, pos, species, cell, nbr, centres=None, max_edges_per_chunk=200_000, taps=None, virial=False):
         """E = sum_i E_i and F_i = -dE/dr_i (B12), using the neighbour list ``nbr`` =
         (rowptr, col, shift).  Edges with r >= r_cut contribute exactly zero and are skipped (A11).
 
         ``centres``: optional array of centre atoms; then only their E_i are summed and F is the
-        gradient of that partial sum (used for subset parity on large configs)."""
+        gradient of that partial sum (used for subset parity on large configs).
+
+        ``virial=True`` appends W[a][b] = -sum_e (rvec_e)_a (g_e)_b [eV] (the stress the
+        paper's tensile test reads, is -W / V, see ``stress``)."""
         pos = np.asarray(pos, dtype=np.float64)
         species = np.asarray(species)
         rowptr, col, shift = nbr
@@ -600,6 +603,7 @@ class AllegroOracle:
         centres = np.arange(N) if centres is None else np.asarray(centres)
         E_atom = np.zeros(N)
         F = np.zeros((N, 3))
+        Wvir = np.zeros((3, 3))
         mu = self.W["mu"]
         k = 0
         while k < centres.size:
@@ -615,7 +619,7 @@ class AllegroOracle:
             dx = (pos[cj] - pos[ci]) + cs * Ld
             d2 = dx[:, 0] * dx[:, 0] + dx[:, 1] * dx[:, 1] + dx[:, 2] * dx[:, 2]
             act = d2 < rc2
-            ci, cj, cs, loc = ci[act], cj[act], cs[act], loc[act]
+            ci, cj, cs, loc, dxa = ci[act], cj[act], cs[act], loc[act], dx[act]
             E_atom[cc] = mu[species[cc]]
             if ci.size:
                 E_i, has, g_e = self._chunk(pos, species, cell, ci, cj, cs, loc, cc.size, taps=taps)
@@ -623,7 +627,10 @@ class AllegroOracle:
                 # B12: F_i = sum_{e in row(i)} g_e - sum_{e: j(e)=i} g_e
                 np.add.at(F, ci, g_e)
                 np.subtract.at(F, cj, g_e)
+                Wvir -= dxa.T @ g_e
             k = k1
+        if virial:
+            return float(np.sum(E_atom[centres])), F, E_atom, Wvir
         return float(np.sum(E_atom[centres])), F, E_atom
 
     def energy(self, pos, species, cell, radius=None):
@@ -633,6 +640,19 @@ class AllegroOracle:
         return self.energy_forces(pos, species, cell, nbr)[0]
 
 
+def stress(virial, cell):
+    """Cauchy stress of the potential part [eV/A^3]: sigma_ab = (1/V) dE/d eps_ab = -W_ab / V for the homogeneous
+    strain r -> (1 + eps) r, cell -> (1 + eps) cell (PAPER.md:69 tensile test, :93/:112 stress in the training loss)."""
+    return -np.asarray(virial) / float(np.prod(_cell_lengths(cell)))
+
+
+def md_deform(pos, cell, cell_new):
+    """A26: affine remap of the (unwrapped) positions from ``cell`` to ``cell_new`` (both orthorhombic):
+    x' = x L'_x / L_x.  The applied strain of PAPER.md:69 is a sequence of such increments between MD segments."""
+    L, Ln = _cell_lengths(cell), _cell_lengths(cell_new)
+    return np.asarray(pos, dtype=np.float64) * (Ln / L), np.diag(Ln)
+
+
 # ================================================================================================
 # a-6: velocity-Verlet NVE with skin-triggered rebuilds                               (A20, A22)
 # ================================================================================================
@@ -640,9 +660,15 @@ def kinetic_energy(vel, mass):
     return float(0.5 * np.sum(mass[:, None] * vel * vel) / ACC_CONV)
 
 
-def md_run(model: AllegroOracle, pos, vel, mass, species, cell, skin, dt, n_steps, neighbor_fn=neighbors_bruteforce):
+def md_run(model: AllegroOracle, pos, vel, mass, species, cell, skin, dt, n_steps, neighbor_fn=neighbors_bruteforce,
+           thermostat=None):
     """Kick-drift-kick; rebuild when max_i |r_i - r_i^build| > skin/2, tested after the drift and
-    before the force call; skin = 0 rebuilds every step.  Returns a dict with the final state."""
+    before the force call; skin = 0 rebuilds every step.  Returns a dict with the final state.
+
+    ``thermostat`` = dict(T0, T1, n_ramp, tau) switches to the canonical ensemble the paper runs (PAPER.md:49,
+    :116 "NVT", :75 heating 300 -> 1200 K), reading A25: Berendsen weak coupling applied after the second half-kick
+    of step k (1-based): T_inst = 2 E_kin / ((3N - 3) k_B), T_target = T0 + (T1 - T0) min(1, k / n_ramp),
+    v <- v sqrt(1 + (dt / tau) (T_target / T_inst - 1))."""
     pos, vel = np.array(pos, dtype=np.float64), np.array(vel, dtype=np.float64)
     radius = model.hp["r_cut"] + skin
     nbr = neighbor_fn(pos, cell, radius)
@@ -661,6 +687,12 @@ def md_run(model: AllegroOracle, pos, vel, mass, species, cell, skin, dt, n_step
             n_rebuilds += 1
         E, F, _ = model.energy_forces(pos, species, cell, nbr)
         vel += 0.5 * dt * ACC_CONV * F / mass[:, None]
+        if thermostat is not None:
+            k = len(traj_E)                                   # 1-based step index
+            T_inst = 2.0 * kinetic_energy(vel, mass) / ((3 * pos.shape[0] - 3) * KB_EV)
+            frac = min(1.0, k / thermostat["n_ramp"]) if thermostat.get("n_ramp", 0) > 0 else 1.0
+            T_tgt = thermostat["T0"] + (thermostat["T1"] - thermostat["T0"]) * frac
+            vel *= math.sqrt(1.0 + (dt / thermostat["tau"]) * (T_tgt / T_inst - 1.0))
         traj_E.append((E, kinetic_energy(vel, mass)))
     return dict(pos=pos, vel=vel, F=F, E_pot=E, E_kin=kinetic_energy(vel, mass), n_rebuilds=n_rebuilds,
                 energies=np.array(traj_E))
