@@ -96,6 +96,23 @@ int allegro_md_init(void* h, const double* pos, const double* vel, const double*
                     int64_t N, const double* cell, double cutoff, double skin, void* stream);
 int allegro_md_step(void* h, double dt_fs, int64_t n_steps, void* stream);
 
+/* the protocols the paper runs (NVT at 300 K: PAPER.md:49, :116; heating 300 -> 1200 K: :75; tensile strain
+ * at fixed rates: :69).  PAPER.md names no thermostat and no deformation scheme; readings A25 / A26:
+ *  - allegro_md_step_nvt: velocity-Verlet as allegro_md_step plus Berendsen weak coupling after the second half-kick of step
+ *    k = 1..n_steps of this call: T_inst = 2 E_kin / ((3N-3) kB), T_target = T0 + (T1-T0) min(1, k/n_ramp) (n_ramp = 0: T1 at
+ *    once), v <- v sqrt(1 + (dt/tau)(T_target/T_inst - 1)).  tau_fs >= dt_fs.  Deterministic; no host sync in the loop.
+ *  - allegro_md_deform: affine remap of the unwrapped positions to cell_new (HOST fp64 [3,3], orthorhombic), x' = x L'/L, full
+ *    list rebuild and force evaluation.  A strain rate is a sequence of such increments between allegro_md_step calls.
+ *  - allegro_set_state: checkpoint / resume — new pos, vel (DEVICE fp64 [N,3]) for the masses, species and cell given to
+ *    allegro_md_init; rebuilds the list and the forces (NVE is deterministic given this state).
+ *  - allegro_virial: W[a][b] = -sum_e (rvec_e)_a (dE/d rvec_e)_b [eV] (DEVICE fp64 [9], row-major) from the per-edge gradients
+ *    of the LAST force evaluation, with pos (DEVICE) the positions of that evaluation or NULL for the MD state.  The potential
+ *    part of the stress is -W / V.  Fixed-order fp64 reduction (deterministic). */
+int allegro_md_step_nvt(void* h, double dt_fs, int64_t n_steps, double T0, double T1, int64_t n_ramp, double tau_fs, void* stream);
+int allegro_md_deform(void* h, const double* cell_new, void* stream);
+int allegro_set_state(void* h, const double* pos, const double* vel, void* stream);
+int allegro_virial(void* h, const double* pos, double* W_out, void* stream);
+
 /* Copies the MD state out.  pos/vel/F DEVICE fp64 [N,3]; E_pot/E_kin DEVICE fp64 [1]; n_rebuilds HOST
  * int64 [1].  Any pointer may be NULL. */
 int allegro_get_state(void* h, double* pos, double* vel, double* F, double* E_pot, double* E_kin,
@@ -108,7 +125,9 @@ int allegro_get_neighbors(void* h, int64_t* rowptr, int32_t* col, int8_t* shift,
 /* Counters of the last energy_forces / md_step call (HOST int64 [8]): [0] active edges (r < r_cut) of
  * the last force evaluation, [1] list edges, [2] kernel launches of the call, [3] rebuilds of the call,
  * [4] force evaluations of the call, [5] atom chunks per force evaluation (the activation workspace is sized from the
- * free device memory; chunks are exact because the model is strictly local), [6..7] reserved. */
+ * free device memory; chunks are exact because the model is strictly local), [6] capacity recoveries of the last md_step (a
+ * device-side rebuild outgrew the list: the integrator halts, the host regrows the list and finishes the call — same
+ * trajectory), [7] reserved. */
 int allegro_get_stats(void* h, int64_t* stats);
 
 /* Per-kernel-class timing for bench.py's roofline line.  allegro_profile(h, 1) resets the counters and makes
@@ -134,6 +153,8 @@ int allegro_debug_num_paths(const allegro_hparams* hp, int layer);
  * A0 / A1 hold rows_cap >= M rows; geo is the [M][8] edge record (u at [4]) or NULL.  Synchronises the stream.
  * Returns ALLEGRO_ERR_UNSUPPORTED when the shape or alignment is outside what the kernel takes. */
 int allegro_debug_set_precision(void* h, int passes);
+/* Test hook: capacity of the next list builds = E + frac * E + extra (default 0.125, 4096); (0, 0) forces the recovery path. */
+int allegro_debug_set_list_slack(void* h, double frac, int64_t extra);
 int allegro_debug_gemm(void* h, int64_t M, int64_t rows_cap, const float* A0, int lda0, int K0, const float* A1, int lda1, int K1,
                        const float* W, int ldw, int wtrans, int N, int pro, int epi, const float* aux, int ldaux, const float* geo,
                        float* C, int ldc, float* C2, int ldc2, int split, float c_old, float c_new, void* stream);

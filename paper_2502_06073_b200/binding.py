@@ -23,7 +23,8 @@ _lib = C.CDLL(LIB_PATH)
 ERR_NAMES = {0: "OK", -1: "INVALID", -2: "UNSUPPORTED", -3: "CUDA", -4: "STALE_LIST", -5: "NONFINITE", -6: "CUTOFF",
              -7: "SPECIES", -8: "NO_LIST", -9: "ALLOC"}
 EXPORTS = ["allegro_weight_layout", "allegro_create", "allegro_destroy", "allegro_build_neighbors",
-           "allegro_energy_forces", "allegro_md_init", "allegro_md_step", "allegro_get_state",
+           "allegro_energy_forces", "allegro_md_init", "allegro_md_step", "allegro_md_step_nvt", "allegro_md_deform",
+           "allegro_set_state", "allegro_virial", "allegro_debug_set_list_slack", "allegro_get_state",
            "allegro_get_neighbors", "allegro_get_stats", "allegro_profile", "allegro_get_profile",
            "allegro_debug_coupling", "allegro_debug_num_paths", "allegro_debug_set_precision", "allegro_debug_gemm",
            "allegro_last_error"]
@@ -54,6 +55,11 @@ _lib.allegro_build_neighbors.argtypes = [_vp, _vp, _vp, _i64, _vp, _dbl, _dbl, _
 _lib.allegro_energy_forces.argtypes = [_vp, _vp, _vp, _i64, _vp, _vp, _vp, _vp, _vp]
 _lib.allegro_md_init.argtypes = [_vp, _vp, _vp, _vp, _vp, _i64, _vp, _dbl, _dbl, _vp]
 _lib.allegro_md_step.argtypes = [_vp, _dbl, _i64, _vp]
+_lib.allegro_md_step_nvt.argtypes = [_vp, _dbl, _i64, _dbl, _dbl, _i64, _dbl, _vp]
+_lib.allegro_md_deform.argtypes = [_vp, _vp, _vp]
+_lib.allegro_set_state.argtypes = [_vp, _vp, _vp, _vp]
+_lib.allegro_virial.argtypes = [_vp, _vp, _vp, _vp]
+_lib.allegro_debug_set_list_slack.argtypes = [_vp, _dbl, _i64]
 _lib.allegro_get_state.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.allegro_get_neighbors.argtypes = [_vp, _vp, _vp, _vp, _vp]
 _lib.allegro_get_stats.argtypes = [_vp, _vp]
@@ -175,6 +181,26 @@ class Allegro:
     def md_step(self, dt_fs, n_steps):
         self._check(_lib.allegro_md_step(self._h, float(dt_fs), int(n_steps), _stream()))
 
+    def md_step_nvt(self, dt_fs, n_steps, T0, T1, n_ramp, tau_fs):
+        self._check(_lib.allegro_md_step_nvt(self._h, float(dt_fs), int(n_steps), float(T0), float(T1), int(n_ramp), float(tau_fs), _stream()))
+
+    def md_deform(self, cell_new):
+        c = self._cell_host(cell_new)
+        self._check(_lib.allegro_md_deform(self._h, c.ctypes.data, _stream()))
+
+    def set_state(self, pos, vel):
+        self._check(_lib.allegro_set_state(self._h, _ptr(pos), _ptr(vel), _stream()))
+
+    def virial(self, pos=None):
+        """-> numpy [3,3]; pos = the positions of the last force evaluation (torch CUDA fp64) or None for the MD state."""
+        import torch
+        W = torch.zeros(9, dtype=torch.float64, device="cuda")
+        self._check(_lib.allegro_virial(self._h, _ptr(pos), _ptr(W), _stream()))
+        return W.cpu().numpy().reshape(3, 3)
+
+    def debug_set_list_slack(self, frac, extra):
+        self._check(_lib.allegro_debug_set_list_slack(self._h, float(frac), int(extra)))
+
     def get_state(self, pos=None, vel=None, F=None, E_pot=None, E_kin=None):
         nreb = C.c_int64(0)
         self._check(_lib.allegro_get_state(self._h, _ptr(pos), _ptr(vel), _ptr(F), _ptr(E_pot), _ptr(E_kin),
@@ -198,7 +224,7 @@ class Allegro:
         s = np.zeros(8, np.int64)
         self._check(_lib.allegro_get_stats(self._h, s.ctypes.data))
         return dict(active_edges=int(s[0]), list_edges=int(s[1]), launches=int(s[2]), rebuilds=int(s[3]),
-                    force_evals=int(s[4]), chunks=max(1, int(s[5])))
+                    force_evals=int(s[4]), chunks=max(1, int(s[5])), recoveries=int(s[6]))
 
     def profile(self, enable: bool):
         self._check(_lib.allegro_profile(self._h, 1 if enable else 0))

@@ -16,6 +16,7 @@ static thread_local std::string g_create_err;
 int ensure(Model* m, DevBuf* b, size_t bytes) {
   if (bytes <= b->bytes && b->p) return 0;
   if (b->p) { cudaFree(b->p); b->p = nullptr; b->bytes = 0; }
+  md_graph_reset(m);   // a captured MD step holds the old pointer
   bytes = (bytes + 255) / 256 * 256;
   cudaError_t e = cudaMalloc(&b->p, bytes);
   if (e != cudaSuccess) {
@@ -238,7 +239,7 @@ int allegro_destroy(void* h) {
   NeighborList& nl = m->nl;
   for (DevBuf* b : {&nl.r_build, &nl.img, &nl.cell_of, &nl.cell_cnt, &nl.cell_start, &nl.cell_fill, &nl.sorted, &nl.row_cnt, &nl.rowptr,
                     &nl.keys_tmp, &nl.keys, &nl.revpos, &nl.scan_tmp, &m->ws.arena, &m->ws.scan_tmp, &m->g_list, &m->e_atom, &m->e_partial, &m->act_total,
-                    &m->flags, &m->md_pos, &m->md_vel, &m->md_mass, &m->md_species, &m->md_F, &m->md_E})
+                    &m->flags, &m->md_pos, &m->md_vel, &m->md_mass, &m->md_species, &m->md_F, &m->md_E, &m->vir_partial, &m->nvt_par, &nl.rowptr_new})
     free_buf(*b);
   delete m;
   return ALLEGRO_OK;
@@ -278,6 +279,7 @@ int allegro_energy_forces(void* h, const double* pos, const int32_t* species, in
   int64_t act = 0;
   if (N > 0 && m->act_total.p) cudaMemcpyAsync(&act, m->act_total.p, sizeof(int64_t), cudaMemcpyDeviceToHost, st);
   rc = check_flags(m, st, "allegro_energy_forces");
+  if (rc == ALLEGRO_ERR_ALLOC) { m->ws.slack *= 1.5; m->ws.for_N = -1; }   // a chunk overflowed its workspace share: a retry gets more
   m->stats[0] = act; m->stats[2] = m->launches; m->stats[3] = 0; m->stats[4] = 1;
   return rc;
 }
@@ -299,16 +301,19 @@ int allegro_md_init(void* h, const double* pos, const double* vel, const double*
   return rc;
 }
 
-int allegro_md_step(void* h, double dt_fs, int64_t n_steps, void* stream) {
+static int md_step_api(void* h, double dt_fs, int64_t n_steps, const double* nvt, void* stream) {
   if (!h) return ALLEGRO_ERR_INVALID;
   Model* m = static_cast<Model*>(h);
   if (!m->md_ready) { m->err = "allegro_md_step called before allegro_md_init"; return ALLEGRO_ERR_INVALID; }
   if (n_steps < 0 || !(dt_fs > 0.0)) { m->err = "allegro_md_step: bad argument"; return ALLEGRO_ERR_INVALID; }
+  if (nvt && (!(nvt[0] > 0.0) || !(nvt[1] > 0.0) || nvt[2] < 0.0 || !(nvt[3] >= dt_fs))) {
+    m->err = "allegro_md_step_nvt: temperatures must be > 0, n_ramp >= 0, tau >= dt"; return ALLEGRO_ERR_INVALID;
+  }
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   m->launches = 0;
   const int64_t reb0 = m->nl.n_rebuilds;
-  m->stats[4] = 0;
-  int rc = md_step(m, dt_fs, n_steps, st);
+  m->stats[4] = 0; m->stats[6] = 0;
+  int rc = md_step(m, dt_fs, n_steps, nvt, st);
   if (rc) return rc;
   int64_t act = 0, elist = 0;
   if (m->nl.N > 0) {
@@ -319,6 +324,60 @@ int allegro_md_step(void* h, double dt_fs, int64_t n_steps, void* stream) {
   if (m->nl.N > 0) m->nl.E_list = elist;
   m->stats[0] = act; m->stats[1] = m->nl.E_list; m->stats[2] = m->launches; m->stats[3] = m->nl.n_rebuilds - reb0;
   return rc;
+}
+
+int allegro_md_step(void* h, double dt_fs, int64_t n_steps, void* stream) { return md_step_api(h, dt_fs, n_steps, nullptr, stream); }
+
+int allegro_md_step_nvt(void* h, double dt_fs, int64_t n_steps, double T0, double T1, int64_t n_ramp, double tau_fs, void* stream) {
+  const double par[4] = {T0, T1, (double)n_ramp, tau_fs};
+  return md_step_api(h, dt_fs, n_steps, par, stream);
+}
+
+int allegro_md_deform(void* h, const double* cell_new, void* stream) {
+  if (!h) return ALLEGRO_ERR_INVALID;
+  Model* m = static_cast<Model*>(h);
+  if (!m->md_ready || !cell_new) { m->err = "allegro_md_deform: no MD state or null cell"; return ALLEGRO_ERR_INVALID; }
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  m->launches = 0;
+  int rc = md_deform(m, cell_new, st);
+  if (rc) return rc;
+  rc = check_flags(m, st, "allegro_md_deform");
+  m->stats[2] = m->launches;
+  return rc;
+}
+
+int allegro_set_state(void* h, const double* pos, const double* vel, void* stream) {
+  if (!h) return ALLEGRO_ERR_INVALID;
+  Model* m = static_cast<Model*>(h);
+  if (!m->md_ready || !pos || !vel) { m->err = "allegro_set_state: no MD state (call allegro_md_init first) or null argument"; return ALLEGRO_ERR_INVALID; }
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  m->launches = 0;
+  int rc = md_set_state(m, pos, vel, st);
+  if (rc) return rc;
+  rc = check_flags(m, st, "allegro_set_state");
+  m->stats[2] = m->launches;
+  return rc;
+}
+
+int allegro_virial(void* h, const double* pos, double* W_out, void* stream) {
+  if (!h) return ALLEGRO_ERR_INVALID;
+  Model* m = static_cast<Model*>(h);
+  if (!W_out) { m->err = "allegro_virial: null output"; return ALLEGRO_ERR_INVALID; }
+  if (!m->nl.valid) { m->err = "allegro_virial called before a force evaluation"; return ALLEGRO_ERR_NO_LIST; }
+  if (!pos && !m->md_ready) { m->err = "allegro_virial: pos == NULL needs an MD state"; return ALLEGRO_ERR_INVALID; }
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  int rc = network_virial(m, pos ? pos : m->md_pos.as<double>(), W_out, st);
+  if (rc) return rc;
+  cudaError_t e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return cuda_fail(m, e, "allegro_virial");
+  return ALLEGRO_OK;
+}
+
+int allegro_debug_set_list_slack(void* h, double frac, int64_t extra) {
+  if (!h || frac < 0.0 || extra < 0) return ALLEGRO_ERR_INVALID;
+  Model* m = static_cast<Model*>(h);
+  m->nl.slack_frac = frac; m->nl.slack_extra = extra;
+  return ALLEGRO_OK;
 }
 
 int allegro_get_state(void* h, double* pos, double* vel, double* F, double* E_pot, double* E_kin, int64_t* n_rebuilds, void* stream) {

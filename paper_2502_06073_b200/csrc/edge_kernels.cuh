@@ -39,9 +39,9 @@ __global__ void k_check_inputs(const double* __restrict__ pos, const double* __r
                                int64_t N, double half_skin2, int n_species, int* flags) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= N) return;
-  double dx = pos[3 * i] - r_build[3 * i], dy = pos[3 * i + 1] - r_build[3 * i + 1], dz = pos[3 * i + 2] - r_build[3 * i + 2];
-  double d2 = dx * dx + dy * dy + dz * dz;
-  if (d2 > half_skin2) flags[FLAG_STALE] = 1;
+  const double dx = __dsub_rn(pos[3 * i], r_build[3 * i]), dy = __dsub_rn(pos[3 * i + 1], r_build[3 * i + 1]), dz = __dsub_rn(pos[3 * i + 2], r_build[3 * i + 2]);
+  const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));   // as the oracle: no FMA contraction
+  if (d2 > half_skin2 && !flags[FLAG_HALT]) flags[FLAG_STALE] = 1;   // halted integrator: the host rebuilds and redoes this evaluation
   int z = species[i];
   if (z < 0 || z >= n_species) flags[FLAG_SPECIES] = 1;
 }
@@ -93,13 +93,24 @@ __global__ void k_active(const double* __restrict__ pos, const int* __restrict__
           const double pref = 2.0 / rc * inv * u, w = 3.14159265358979323846 * x;
           for (int n = 1; n <= n_bessel; ++n) bes[dst * n_bessel + (n - 1)] = (float)(pref * sin(n * w));
         } else {
-          flags[FLAG_ERR_CAP] = 2;
+          flags[FLAG_ERR_CAP] = 2;   // unreachable after k_ws_check / k_ws_clamp; kept as a guard
         }
       }
     }
     total += __popc(bal);
   }
   if (MODE == 0 && lane == 0) act_cnt[a - a0] = total;
+}
+
+// Activation-workspace guard: when the chunk holds more active edges than the workspace, the chunk is emptied (every row
+// offset 0: all edge kernels see M = 0 and do nothing), the error is flagged and the integrator halted; the host re-sizes.
+__global__ void k_ws_check(const int64_t* rowptr_c, int64_t na, int64_t cap_edges, int* flags) {
+  if (rowptr_c[na] > cap_edges) { flags[FLAG_ERR_CAP] = 2; flags[FLAG_HALT] = 1; }
+}
+__global__ void k_ws_clamp(int64_t* rowptr_c, int64_t na, const int* flags) {
+  if (flags[FLAG_ERR_CAP] != 2) return;
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i <= na) rowptr_c[i] = 0;
 }
 
 // F7: Gamma_i[lm, c] = Nbar^-1/2 sum_{e in row(i)} w[e, l, c] Y_lm(rhat_e).  One block per centre atom.  A thread owns a
@@ -388,6 +399,45 @@ __global__ void k_force_gather(ListView lv, int64_t N, const float* __restrict__
     F[3 * i] = fx; F[3 * i + 1] = fy; F[3 * i + 2] = fz;
     if (!(isfinite(fx) && isfinite(fy) && isfinite(fz))) flags[FLAG_NONFINITE] = 1;
   }
+}
+
+// Virial W[a][b] = -sum_e (rvec_e)_a (g_e)_b over the list edges (g = 0 on inactive ones); rvec_e in fp64 with
+// the expression of the list criterion.  Warps stride over the atoms, lanes over a row; fixed-shape reduction: lane tree,
+// warp partials in shared memory, block partials [gridDim.x][9], then k_virial_final (one block) — deterministic, no atomics.
+__global__ void __launch_bounds__(256) k_virial_partial(ListView lv, const double* __restrict__ pos, int64_t N, const float* __restrict__ g_list,
+                                                        double* __restrict__ partial) {
+  __shared__ double sh[8][9];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  double w[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+  for (int64_t i = (int64_t)blockIdx.x * 8 + warp; i < N; i += (int64_t)gridDim.x * 8) {
+    for (int64_t k = lv.rowptr[i] + lane; k < lv.rowptr[i + 1]; k += 32) {
+      double d[3]; int j;
+      edge_d2(pos, i, lv.keys[k], lv.L, &d[0], &d[1], &d[2], &j);
+      const double g[3] = {(double)g_list[3 * k], (double)g_list[3 * k + 1], (double)g_list[3 * k + 2]};
+#pragma unroll
+      for (int a = 0; a < 3; ++a)
+#pragma unroll
+        for (int b = 0; b < 3; ++b) w[3 * a + b] -= d[a] * g[b];
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < 9; ++q) {
+#pragma unroll
+    for (int dd = 16; dd > 0; dd >>= 1) w[q] += __shfl_xor_sync(0xffffffffu, w[q], dd);
+    if (lane == 0) sh[warp][q] = w[q];
+  }
+  __syncthreads();
+  if (threadIdx.x < 9) {
+    double s = 0;
+    for (int ww = 0; ww < 8; ++ww) s += sh[ww][threadIdx.x];
+    partial[(int64_t)blockIdx.x * 9 + threadIdx.x] = s;
+  }
+}
+__global__ void k_virial_final(const double* __restrict__ partial, int nb, double* __restrict__ W) {
+  if (threadIdx.x >= 9) return;
+  double s = 0;
+  for (int b = 0; b < nb; ++b) s += partial[(int64_t)b * 9 + threadIdx.x];
+  W[threadIdx.x] = s;
 }
 
 // E = sum_i E_i in fp64: fixed-shape two-stage tree (deterministic)

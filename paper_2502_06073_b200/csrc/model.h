@@ -40,11 +40,14 @@ struct NeighborList {
   int64_t E_list = 0, cap = 0;
   int64_t n_rebuilds = 0;
   DevBuf r_build, img, cell_of, cell_cnt, cell_start, cell_fill, sorted, row_cnt, rowptr, keys_tmp, keys, revpos;
-  DevBuf scan_tmp;
+  DevBuf scan_tmp, rowptr_new;
+  double slack_frac = 0.125; int64_t slack_extra = 4096;   // list capacity beyond the count of the sizing build
 };
 
 struct Workspace {       // per-chunk activations, sized for cap_edges active edges and cap_atoms atoms
   int64_t cap_edges = 0, cap_atoms = 0;
+  int64_t for_N = -1, for_cap = -1, atoms_per = 0;   // chunking decided for this (N, list capacity); kept while it fits
+  double slack = 1.25;                                  // active edges of a chunk allowed over the average list row
   DevBuf arena;          // one allocation, carved below
   // chunk-local CSR of active edges
   int* act_cnt = nullptr; int64_t* rowptr_c = nullptr; DevBuf scan_tmp;
@@ -100,13 +103,14 @@ struct Model {
   NeighborList nl;
   Workspace ws;
   // global per-list-edge gradient and per-atom outputs
-  DevBuf g_list, e_atom, e_partial, act_total, flags, md_pos, md_vel, md_mass, md_species, md_F, md_E;
+  DevBuf g_list, e_atom, e_partial, act_total, flags, md_pos, md_vel, md_mass, md_species, md_F, md_E, vir_partial, nvt_par;
   bool md_ready = false;
   // CUDA-graph replay of one MD step (md.cu)
   bool use_graph = true, md_warm = false;
   cudaStream_t own_stream = nullptr, graph_stream = nullptr;
   cudaGraphExec_t md_graph = nullptr;
   double graph_dt = 0;
+  int graph_nvt = 0;
   int64_t graph_launches = 0;
   double md_cell[9] = {0};
   int64_t stats[8] = {0};
@@ -115,7 +119,9 @@ struct Model {
 
 // device flag slots (int32 array in Model::flags)
 enum { FLAG_REBUILD = 0, FLAG_ERR_SHIFT = 1, FLAG_ERR_CAP = 2, FLAG_STALE = 3, FLAG_NONFINITE = 4, FLAG_SPECIES = 5,
-       FLAG_NREBUILD = 6, FLAG_COUNT = 16 };
+       FLAG_NREBUILD = 6, FLAG_HALT = 7, FLAG_STEPS = 8, FLAG_COUNT = 16 };
+// FLAG_HALT: a device-side rebuild (or the activation workspace) ran out of capacity: the integrator kernels of the remaining
+// steps of the call do nothing, FLAG_STEPS counts the completed steps, the host regrows and finishes the call (md.cu).
 
 // ---- profiling brackets (api.cu)
 void prof_begin(Model* m, cudaStream_t st, int cls, double work);
@@ -141,7 +147,10 @@ int network_energy_forces(Model* m, const double* pos, const int32_t* species, i
 // ---- md.cu
 int md_init(Model* m, const double* pos, const double* vel, const double* mass, const int32_t* species, int64_t N,
             const double* cell, double cutoff, double skin, cudaStream_t st);
-int md_step(Model* m, double dt, int64_t n_steps, cudaStream_t st);
+int md_step(Model* m, double dt, int64_t n_steps, const double* nvt /*[4] T0, T1, n_ramp, tau or NULL*/, cudaStream_t st);
+int md_deform(Model* m, const double* cell_new, cudaStream_t st);
+int md_set_state(Model* m, const double* pos, const double* vel, cudaStream_t st);
+int network_virial(Model* m, const double* pos, double* W_out, cudaStream_t st);
 int md_kinetic(Model* m, double* Ekin_dev, cudaStream_t st);
 void md_graph_reset(Model* m);
 

@@ -218,9 +218,16 @@ __global__ void k_nbr_pass(const double* __restrict__ pos, int64_t N, Grid g, do
   if (MODE == 0 && lane == 0) row_cnt[i] = total;
 }
 
-__global__ void k_check_cap(const int64_t* rowptr, int64_t N, int64_t cap, int* flags) {
+// The new row offsets are scanned into a scratch array: when the rebuilt list would not fit, the old list (offsets included)
+// stays intact, the rebuild is cancelled and the integrator is halted (FLAG_HALT); the host regrows and finishes the call.
+__global__ void k_check_cap(const int64_t* rowptr_new, int64_t N, int64_t cap, int* flags) {
   if (flags[FLAG_REBUILD] == 0) return;
-  if (rowptr[N] > cap) atomicExch(&flags[FLAG_ERR_CAP], 1);
+  if (rowptr_new[N] > cap) { flags[FLAG_ERR_CAP] = 1; flags[FLAG_HALT] = 1; flags[FLAG_REBUILD] = 0; }
+}
+__global__ void k_commit_rowptr(const int64_t* __restrict__ rowptr_new, int64_t* __restrict__ rowptr, int64_t N, const int* flags) {
+  if (flags[FLAG_REBUILD] == 0) return;
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i <= N) rowptr[i] = rowptr_new[i];
 }
 
 // One warp per row: rank of each key among the row's keys (keys are distinct) -> sorted position.
@@ -320,6 +327,7 @@ int nl_build(Model* m, const double* pos, int64_t N, const double* cell, double 
     rc |= ensure(m, &nl.sorted, sizeof(int) * N + 8);
     rc |= ensure(m, &nl.row_cnt, sizeof(int) * N + 8);
     rc |= ensure(m, &nl.rowptr, sizeof(int64_t) * (N + 1));
+    rc |= ensure(m, &nl.rowptr_new, sizeof(int64_t) * (N + 1));
     if (rc) return ALLEGRO_ERR_ALLOC;
     int one = 1;
     cudaMemcpyAsync(&flags[FLAG_REBUILD], &one, sizeof(int), cudaMemcpyHostToDevice, st);
@@ -343,15 +351,15 @@ int nl_build(Model* m, const double* pos, int64_t N, const double* cell, double 
   k_bin_scatter<<<gridN, T, 0, st>>>(N, nl.cell_of.as<int>(), nl.cell_start.as<int64_t>(), nl.cell_fill.as<int>(), nl.sorted.as<int>(), flags);
   k_nbr_pass<0><<<gridW, T, 0, st>>>(pos, N, g, R * R, nl.img.as<int>(), nl.cell_of.as<int>(), nl.cell_start.as<int64_t>(),
                                      nl.sorted.as<int>(), nl.row_cnt.as<int>(), nullptr, nullptr, 0, flags);
-  if (int rc = scan_counts(m, nl.row_cnt.as<int>(), nl.rowptr.as<int64_t>(), N, &nl.scan_tmp, &flags[FLAG_REBUILD], st)) return rc;
+  if (int rc = scan_counts(m, nl.row_cnt.as<int>(), nl.rowptr_new.as<int64_t>(), N, &nl.scan_tmp, &flags[FLAG_REBUILD], st)) return rc;
   m->launches += 3;
   if (!conditional) {
     int64_t E = 0;
-    cudaMemcpyAsync(&E, nl.rowptr.as<int64_t>() + N, sizeof(int64_t), cudaMemcpyDeviceToHost, st);
+    cudaMemcpyAsync(&E, nl.rowptr_new.as<int64_t>() + N, sizeof(int64_t), cudaMemcpyDeviceToHost, st);
     cudaError_t e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) return cuda_fail(m, e, "neighbor count pass");
     nl.E_list = E;
-    int64_t cap = E + E / 8 + 4096;   // slack for the conditional rebuilds of the MD loop
+    int64_t cap = E + (int64_t)(nl.slack_frac * (double)E) + nl.slack_extra;   // slack for the conditional rebuilds of the MD loop
     int rc = 0;
     rc |= ensure(m, &nl.keys_tmp, sizeof(uint64_t) * cap);
     rc |= ensure(m, &nl.keys, sizeof(uint64_t) * cap);
@@ -361,7 +369,8 @@ int nl_build(Model* m, const double* pos, int64_t N, const double* cell, double 
     nl.cap = std::min<int64_t>({(int64_t)(nl.keys.bytes / 8), (int64_t)(nl.keys_tmp.bytes / 8), (int64_t)(nl.revpos.bytes / 4),
                                 (int64_t)(m->g_list.bytes / 12)});
   }
-  k_check_cap<<<1, 1, 0, st>>>(nl.rowptr.as<int64_t>(), N, nl.cap, flags);
+  k_check_cap<<<1, 1, 0, st>>>(nl.rowptr_new.as<int64_t>(), N, nl.cap, flags);
+  k_commit_rowptr<<<(unsigned)((N + 1 + T - 1) / T), T, 0, st>>>(nl.rowptr_new.as<int64_t>(), nl.rowptr.as<int64_t>(), N, flags);
   k_nbr_pass<1><<<gridW, T, 0, st>>>(pos, N, g, R * R, nl.img.as<int>(), nl.cell_of.as<int>(), nl.cell_start.as<int64_t>(),
                                      nl.sorted.as<int>(), nullptr, nl.rowptr.as<int64_t>(), nl.keys_tmp.as<uint64_t>(), nl.cap, flags);
   k_row_sort<<<gridW, T, 0, st>>>(N, nl.rowptr.as<int64_t>(), nl.keys_tmp.as<uint64_t>(), nl.keys.as<uint64_t>(), nl.cap, flags);

@@ -160,11 +160,13 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
   k_active<0><<<gridWA, T, 0, st>>>(pos, species, lv, a0, a1, hp.r_cut, hp.poly_p, Nb, ws.act_cnt, nullptr, nullptr, nullptr, nullptr,
                                     nullptr, nullptr, nullptr, 0, flags);
   if (int rc = scan_counts(m, ws.act_cnt, ws.rowptr_c, na, &ws.scan_tmp, nullptr, st)) return rc;
+  k_ws_check<<<1, 1, 0, st>>>(ws.rowptr_c, na, ws.cap_edges, flags);
+  k_ws_clamp<<<(unsigned)((na + 1 + T - 1) / T), T, 0, st>>>(ws.rowptr_c, na, flags);
   k_active<1><<<gridWA, T, 0, st>>>(pos, species, lv, a0, a1, hp.r_cut, hp.poly_p, Nb, nullptr, ws.rowptr_c, ws.e_center, ws.e_j,
                                     ws.e_lidx, ws.geo, ws.bes, m->g_list.as<float>(), ws.cap_edges, flags);
   k_add_count<<<1, 1, 0, st>>>(ws.rowptr_c + na, m->act_total.as<int64_t>());
   prof_end(m, st);
-  m->launches += 3;
+  m->launches += 5;
   const int64_t* Mptr = ws.rowptr_c + na;
   const float* w = m->d_w;
   const unsigned gridE = (unsigned)((m_cap + T - 1) / T), gridWE = (unsigned)((m_cap * 32 + T - 1) / T);
@@ -469,18 +471,24 @@ int network_energy_forces(Model* m, const double* pos, const int32_t* species, i
     k_check_inputs<<<(unsigned)((N + T - 1) / T), T, 0, st>>>(pos, nl.r_build.as<double>(), species, N, hs * hs, m->plan.hp.n_species, flags);
     m->launches += 1;
   }
-  // single chunk when the workspace fits; otherwise atom chunks bounded by list edges (sized with the average row)
-  size_t pe, pa;
-  ws_sizes(m->plan, m->use_big, &pe, &pa);
-  size_t free_b = 0, total_b = 0;
-  cudaMemGetInfo(&free_b, &total_b);
-  const size_t budget = (size_t)(0.80 * (double)(free_b + m->ws.arena.bytes));
-  int64_t n_chunks = 1;
+  // single chunk when the workspace fits; otherwise atom chunks bounded by list edges (sized with the average row).  The
+  // decision is taken once per (N, list capacity) and kept, so that a captured MD step never sees its buffers move.
+  Workspace& ws = m->ws;
   const int64_t Ecap = std::max<int64_t>(nl.cap, 1);
-  while ((pe * (size_t)(Ecap / n_chunks + 1) * 1.25 + pa * (size_t)(N / n_chunks + 1)) > budget && n_chunks < N) n_chunks *= 2;
-  const int64_t atoms_per = (N + n_chunks - 1) / std::max<int64_t>(n_chunks, 1);
-  const int64_t edges_per = (n_chunks == 1) ? Ecap : (int64_t)((double)Ecap / n_chunks * 1.25) + 4096;
-  if (int rc = ws_prepare(m, edges_per, atoms_per)) return rc;
+  if (ws.for_N != N || ws.for_cap != Ecap || !ws.arena.p) {
+    size_t pe, pa;
+    ws_sizes(m->plan, m->use_big, &pe, &pa);
+    size_t free_b = 0, total_b = 0;
+    cudaMemGetInfo(&free_b, &total_b);
+    const size_t budget = (size_t)(0.80 * (double)(free_b + ws.arena.bytes));
+    int64_t n_chunks = 1;
+    while ((pe * (size_t)(Ecap / n_chunks + 1) * ws.slack + pa * (size_t)(N / n_chunks + 1)) > budget && n_chunks < N) n_chunks *= 2;
+    const int64_t atoms_per = (N + n_chunks - 1) / std::max<int64_t>(n_chunks, 1);
+    const int64_t edges_per = (n_chunks == 1) ? Ecap : (int64_t)((double)Ecap / n_chunks * ws.slack) + 4096;
+    if (int rc = ws_prepare(m, edges_per, atoms_per)) return rc;
+    ws.for_N = N; ws.for_cap = Ecap; ws.atoms_per = std::max<int64_t>(atoms_per, 1);
+  }
+  const int64_t atoms_per = ws.atoms_per;
   for (int64_t a0 = 0; a0 < N; a0 += atoms_per) {
     const int64_t a1 = std::min(N, a0 + atoms_per);
     if (int rc = run_chunk(m, pos, species, a0, a1, m->ws.cap_edges, st)) return rc;
@@ -500,6 +508,20 @@ int network_energy_forces(Model* m, const double* pos, const int32_t* species, i
   if (E_atom_out && N > 0) cudaMemcpyAsync(E_atom_out, m->e_atom.p, sizeof(float) * N, cudaMemcpyDeviceToDevice, st);
   m->stats[1] = nl.E_list;
   m->stats[5] = (N + atoms_per - 1) / std::max<int64_t>(atoms_per, 1);   // atom chunks of this force call
+  return 0;
+}
+
+// W = -sum_e rvec_e (x) g_e from the per-edge gradients of the last force evaluation
+int network_virial(Model* m, const double* pos, double* W_out, cudaStream_t st) {
+  NeighborList& nl = m->nl;
+  const int64_t N = nl.N;
+  const int nb = (int)std::max<int64_t>(1, std::min<int64_t>(1024, (N + 7) / 8));
+  if (int rc = ensure(m, &m->vir_partial, sizeof(double) * 9 * 1024)) return rc;
+  ListView lv{nl.rowptr.as<int64_t>(), nl.keys.as<uint64_t>(), nl.revpos.as<int>(), {nl.L[0], nl.L[1], nl.L[2]}};
+  if (N == 0) { cudaMemsetAsync(W_out, 0, sizeof(double) * 9, st); return 0; }
+  k_virial_partial<<<nb, 256, 0, st>>>(lv, pos, N, m->g_list.as<float>(), m->vir_partial.as<double>());
+  k_virial_final<<<1, 32, 0, st>>>(m->vir_partial.as<double>(), nb, W_out);
+  m->launches += 2;
   return 0;
 }
 
