@@ -2,8 +2,10 @@
 """bench.py — energy+force atom-steps/s of the Allegro MD hot path on B200 (BASELINE.json metric).
 
 One "step" = one allegro_md_step(dt, n_md) call = n_md velocity-Verlet steps (neighbour rebuilds on skin
-violation included) of BASELINE.json configs[1] (4,096-atom SiO2-like box, lmax=2, 2 layers, 16 channels)
-unless --config says otherwise.  value = atoms * n_md * steps / device time (CUDA events, max over ranks).
+violation included).  Default workload: BASELINE.json configs[3], the largest single-GPU configuration and the one
+north_star sets the roofline target on (262,144 atoms, lmax=3, 3 layers, 64 channels, 512-wide MLPs), with
+n_md = 1 so that the driver's --steps/--warmup fit its window; --config 0|1|2|4 select the others and --sweep
+runs the configs[4] size sweep.  value = atoms * n_md * steps / device time (CUDA events, max over ranks).
 `e2e` repeats it through the same C-ABI calls with HOST buffers: pinned host -> device copies of the inputs,
 allegro_md_init, allegro_md_step, allegro_get_state and device -> host copies of the results inside the
 timed region.  N > 1 GPUs: independent replicas (the path does not shard in this build).
@@ -28,6 +30,10 @@ sys.path.insert(0, ROOT)
 METRIC = "energy+force atom-steps/s"
 UNIT = "atom-steps/s"
 FP32_LANES_PER_SM = 128
+# MD steps per bench step when --md-steps is not given: sized so that the driver's --steps 20 --warmup 5 stays within minutes
+DEFAULT_MD_STEPS = {0: 10, 1: 100, 2: 10, 3: 1, 4: 10}
+# centre atoms of one oracle evaluation in the cpu_baseline / reference legs (seconds of host work, bounded memory)
+ORACLE_SAMPLE = {0: 64, 1: 512, 2: 256, 3: 96, 4: 512}
 
 
 def parse():
@@ -36,7 +42,8 @@ def parse():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--sweep", default="", help="configs[4] size sweep: comma-separated log2 N (e.g. 15,17,19,21,23)")
     ap.add_argument("--log2n", type=int, default=15, help="size for --config 4")
     ap.add_argument("--md-steps", type=int, default=0, help="MD steps per bench step (default: the config's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -47,7 +54,7 @@ def parse():
 def load_workload(args):
     from paper_2502_06073_b200 import workloads as WL
     w = WL.get(args.config, log2_n=args.log2n) if args.config == 4 else WL.get(args.config)
-    n_md = args.md_steps or w.n_steps
+    n_md = args.md_steps or DEFAULT_MD_STEPS[args.config]
     return WL, w, n_md
 
 
@@ -56,7 +63,8 @@ def config_dict(w, n_md, extra=None):
     d = {"workload": w.name, "n_atoms": w.n_atoms, "md_steps_per_step": n_md, "dt_fs": w.dt_fs, "skin": w.skin,
          "r_cut": hp["r_cut"], "lmax": hp["lmax"], "n_layers": hp["n_layers"], "n_channels": hp["n_channels"],
          "latent": hp["latent_dims"], "two_body": hp["two_body_dims"], "notes": w.notes,
-         "cache": "inputs larger than L2: the per-step activation working set (about 1.4 GB for cfg 1) exceeds the 126 MB L2; no explicit flush"}
+         "cache": "inputs larger than L2: every MD step streams its activation working set (GBs; >= 1.4 GB already for cfg 1) "
+                  "through the 126 MB L2, so no step starts warm; no explicit flush"}
     if extra:
         d.update(extra)
     return d
@@ -80,13 +88,17 @@ def oracle_time_sample(w, model, nbr, centres):
     return time.perf_counter() - t0
 
 
-def cores_used():
-    try:
-        import threadpoolctl
-        n = max([p["num_threads"] for p in threadpoolctl.threadpool_info()] + [1])
-    except Exception:
-        n = 1
-    return min(n, len(os.sched_getaffinity(0)))
+class CpuMeter:
+    """Average number of busy threads of this process between start() and stop() (user + system CPU time / wall time)."""
+
+    def start(self):
+        self.t0, self.c0 = time.perf_counter(), sum(os.times()[:2])
+        return self
+
+    def stop(self):
+        wall = time.perf_counter() - self.t0
+        cpu = sum(os.times()[:2]) - self.c0
+        return max(1, int(round(cpu / max(wall, 1e-9)))), wall
 
 
 def run_reference(args):
@@ -96,11 +108,13 @@ def run_reference(args):
     WL, w, n_md = load_workload(args)
     O, model, nbr = oracle_setup(w)
     rng = np.random.default_rng(123)
-    ns = args.sample_atoms or min(w.n_atoms, 512)
+    ns = args.sample_atoms or min(w.n_atoms, ORACLE_SAMPLE[args.config])
     centres = np.sort(rng.choice(w.n_atoms, ns, replace=False))
     for _ in range(args.warmup):
         oracle_time_sample(w, model, nbr, centres)
+    meter = CpuMeter().start()
     t = [oracle_time_sample(w, model, nbr, centres) for _ in range(args.steps)]
+    cores, _ = meter.stop()
     tot = sum(t)
     val = ns * args.steps / tot
     sample = (f"each step = one oracle energy+force evaluation (fp64 numpy) for {ns} seeded centre atoms of {w.name} "
@@ -108,7 +122,8 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * tot / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": config_dict(w, n_md),
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores_used(), "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "cores_available": len(os.sched_getaffinity(0)),
+                             "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -170,46 +185,63 @@ def whole_job_value(world, n_atoms, n_md, steps, ms):
     return world * n_atoms * n_md * steps / (ms * 1e-3)
 
 
-def roofline_for(prof, stats, clocks, peaks, n_sm):
-    """`roofline` object of the JSON line for the dominant kernel class of the profiled step."""
+def roofline_for(prof, stats, clocks, peaks, n_sm, n_atoms, ms_md_step):
+    """`roofline` object of the JSON line: the dominant kernel class of the profiled MD step against the peak of the pipe that
+    bounds it, and the per-step fraction t_roof / t_step of SURVEY.md 8d with its three terms (tensor, FP32 ALU, HBM)."""
     sm_max = (clocks or {}).get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
+    sm_now = (clocks or {}).get("sm_mhz") or sm_max
+    at_max = sm_now >= 0.97 * sm_max
+    # dense 16-bit tensor peak: the burst figure when the SM clock stayed at its maximum over the timed region, else the sustained one
+    t16 = (peaks.get("bf16_tflops") if at_max else peaks.get("bf16_tflops_sustained")) or peaks.get("bf16_tflops_sustained") or 1413.0
+    t16_src = ("MEASURED_PEAKS.json bf16_tflops (burst: clocks.sm stayed at max)" if at_max else
+               "MEASURED_PEAKS.json bf16_tflops_sustained (clocks.sm below max under load)") if peaks else "fallback 1413 TF"
+    peak_f16s = t16 / 3.0                           # split-fp16 product = 3 kind::f16 passes (gemm_f16s.cu; fp16 rate = bf16 rate)
+    peak_tf32x3 = t16 * (1.1 / 2.25) / 3.0          # 3 x TF32 passes (gemm_tc.cu); TF32 : BF16 nominal ratio of the guide
     fp32_peak = n_sm * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    hbm = peaks.get("hbm_gbs", 6650.0)
     tot_ms = sum(v["ms"] for v in prof.values()) or 1.0
     dom = max(prof, key=lambda k: prof[k]["ms"])
-    E_act = stats["active_edges"]
+    E_act, E_list = stats["active_edges"], stats["list_edges"]
+    chunks = max(1, stats.get("chunks", 1))
     shares = {k: round(v["ms"] / tot_ms, 4) for k, v in prof.items() if v["launches"]}
-    names = {"gemm": "k_gemm_chain", "tp_fwd": "k_tp_fwd3", "tp_bwd": "k_tp_bwd3"}
+    names = {"gemm": "k_gemm_chain", "gemm_f16s": "k_gemm_f16s", "tp_fwd": "k_tp_fwd3 / k_tpo_fwd", "tp_bwd": "k_tp_bwd3 / k_tpo_bwd"}
     roof = {"kernel": names.get(dom, dom), "shares": shares}
-    traffic = None
+    flops = {k: prof[k]["work"] * E_act / chunks for k in ("gemm", "gemm_f16s", "tp_fwd", "tp_bwd") if k in prof}
+    traffic, traffic_src = None, None
     try:
-        tr = json.load(open(os.path.join(ROOT, "profiles", "r1_traffic.json")))
-        traffic = tr.get(roof["kernel"], {}).get("dram_bytes_per_launch")
+        tr = json.load(open(os.path.join(ROOT, "profiles", "r2_traffic.json")))
+        ent = tr.get(roof["kernel"], {})
+        traffic, traffic_src = ent.get("dram_bytes_per_launch"), ent.get("source")
     except Exception:
         pass
-    if dom in ("gemm", "tp_fwd", "tp_bwd"):
-        # algorithmic flop of all launches of the class: `work` sums flop per edge over launches, and every launch
-        # covers one atom chunk, i.e. active_edges / chunks edges on average
-        flops = prof[dom]["work"] * E_act / max(1, stats.get("chunks", 1))
-        ach = flops / (prof[dom]["ms"] * 1e-3) / 1e12
-        common = {"achieved": ach, "unit": "TFLOP/s", "traffic": traffic, "launches": prof[dom]["launches"],
-                  "avg_launch_ms": prof[dom]["ms"] / max(1, prof[dom]["launches"]),
-                  "algorithmic_flop_per_launch": flops / max(1, prof[dom]["launches"])}
-        if dom == "gemm":
-            bf16 = peaks.get("bf16_tflops_sustained") or peaks.get("bf16_tflops") or 1413.0
-            tf32 = bf16 * (1.1 / 2.25)                                  # guide's nominal TF32 : BF16 dense ratio
-            peak = tf32 / 3.0                                           # fp32-accurate product = 3 TF32 passes (DESIGN.md)
-            roof.update({"bound": "tensor", "peak": peak, "frac": ach / peak, **common,
-                         "peak_source": ("MEASURED_PEAKS.json bf16_tflops_sustained x 1.1/2.25 (nominal TF32:BF16) / 3 "
-                                         "(3-pass hi/lo TF32 split needed for the 1e-4 x RMS force gate)") if peaks else
-                                        "fallback 1413 TF bf16 sustained x 1.1/2.25 / 3",
-                         "peak_tf32_dense": tf32})
-        else:
-            roof.update({"bound": "alu", "peak": fp32_peak, "frac": ach / fp32_peak, **common,
-                         "peak_source": "148 SM x 128 FP32 lanes x 2 x clocks.max.sm (DESIGN.md)"})
+    if dom in flops:
+        ach = flops[dom] / (prof[dom]["ms"] * 1e-3) / 1e12
+        peak = {"gemm": peak_tf32x3, "gemm_f16s": peak_f16s}.get(dom, fp32_peak)
+        roof.update({"bound": "tensor" if dom.startswith("gemm") else "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+                     "frac": ach / peak, "traffic": traffic, "traffic_source": traffic_src, "launches": prof[dom]["launches"],
+                     "avg_launch_ms": prof[dom]["ms"] / max(1, prof[dom]["launches"]),
+                     "algorithmic_flop_per_launch": flops[dom] / max(1, prof[dom]["launches"]),
+                     "peak_source": {"gemm": t16_src + " x 1.1/2.25 (nominal TF32:BF16) / 3 passes (3xTF32 split, gemm_tc.cu)",
+                                     "gemm_f16s": t16_src + " / 3 passes (split-fp16 product hi*hi + hi*lo + lo*hi, gemm_f16s.cu)"}.get(
+                                         dom, "148 SM x 128 FP32 lanes x 2 x clocks.max.sm (DESIGN.md)")})
     else:
-        hbm = peaks.get("hbm_gbs", 6650.0)
         roof.update({"bound": "hbm", "achieved": None, "peak": hbm, "unit": "GB/s", "frac": None, "traffic": traffic,
                      "peak_source": "MEASURED_PEAKS.json" if peaks else "fallback"})
+    # ---- per MD step: t_roof = max(F_gemm / P_tc, F_alu / P_fp32, B_alg / BW_hbm)   (SURVEY.md 8d)
+    t_tensor = (flops.get("gemm", 0.0) / (peak_tf32x3 * 1e12) + flops.get("gemm_f16s", 0.0) / (peak_f16s * 1e12)) * 1e3
+    t_alu = (flops.get("tp_fwd", 0.0) + flops.get("tp_bwd", 0.0)) / (fp32_peak * 1e12) * 1e3
+    b_alg = 52.0 * n_atoms + 8.0 * E_list + 96.0 * n_atoms
+    t_hbm = b_alg / (hbm * 1e9) * 1e3
+    t_roof = max(t_tensor, t_alu, t_hbm)
+    roof["per_step"] = {"t_step_ms": ms_md_step, "t_roof_ms": t_roof, "frac": t_roof / ms_md_step,
+                        "t_tensor_ms": t_tensor, "t_alu_ms": t_alu, "t_hbm_ms": t_hbm,
+                        "gemm_flop": flops.get("gemm", 0.0) + flops.get("gemm_f16s", 0.0),
+                        "alu_flop": flops.get("tp_fwd", 0.0) + flops.get("tp_bwd", 0.0), "algorithmic_bytes": b_alg,
+                        "peaks": {"tensor_f16_split_tflops": peak_f16s, "tensor_tf32x3_tflops": peak_tf32x3, "fp32_tflops": fp32_peak,
+                                  "hbm_gbs": hbm, "tensor_peak_kind": "burst" if at_max else "sustained"},
+                        "note": "algorithmic flop of one MD step (one force evaluation: forward + input-gradient backward), counted "
+                                "once per product whatever the number of tensor passes; the tensor term uses the peak of the kind "
+                                "each GEMM runs in divided by its passes"}
     return roof
 
 
@@ -316,11 +348,11 @@ def run_ours(args):
         pass
     n_sm = torch.cuda.get_device_properties(local).multi_processor_count
     E_act = stats["active_edges"]
-    roof = roofline_for(prof, stats, clocks, peaks, n_sm)
+    roof = roofline_for(prof, stats, clocks, peaks, n_sm, N, ms / args.steps / n_md)
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32", "data": "synthetic",
+            "dtype": "f32 (dense linears: split-fp16 x3 or TF32 x3 tensor-core products, fp32 accumulation)", "data": "synthetic",
             "config": config_dict(w, n_md, {"parallelism": "replicas" if world > 1 else "single",
                                             "active_edges": E_act, "list_edges": stats["list_edges"],
                                             "rebuilds_in_timed_region": rebuilds}),
@@ -338,24 +370,82 @@ def run_ours(args):
     if not args.no_cpu_baseline:
         O, omodel, nbr = oracle_setup(w)
         rng = np.random.default_rng(123)
-        ns = min(N, 512)
+        ns = min(N, ORACLE_SAMPLE[args.config])
         centres = np.sort(rng.choice(N, ns, replace=False))
-        oracle_time_sample(w, omodel, nbr, centres[:32])
+        oracle_time_sample(w, omodel, nbr, centres[: max(8, ns // 8)])
+        meter = CpuMeter().start()
         reps, tsum = 0, 0.0
         while tsum < 10.0 and reps < 20:
             tsum += oracle_time_sample(w, omodel, nbr, centres); reps += 1
-        line["cpu_baseline"] = {"value": ns * reps / tsum, "unit": UNIT, "cores": cores_used(), "kind": "oracle",
+        cores, _ = meter.stop()
+        line["cpu_baseline"] = {"value": ns * reps / tsum, "unit": UNIT, "cores": cores, "cores_available": len(os.sched_getaffinity(0)),
+                                "kind": "oracle",
                                 "sample": f"{reps} oracle energy+force evaluations (fp64 numpy, as it stands) over {ns} seeded centre "
-                                          f"atoms of {w.name} with their full neighbourhoods, {tsum:.1f} s of CPU work"}
+                                          f"atoms of {w.name} with their full neighbourhoods, {tsum:.1f} s of wall time; cores = CPU time / wall time"}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+
+
+def run_sweep(args):
+    """BASELINE.json configs[4]: the config-1 network on tiled 2.2 g/cc SiO2-like boxes, N = 2^k.  One JSON line with one entry per
+    size (atom-steps/s, ms per MD step, per-step roofline fraction, device memory in use); sizes that do not fit end the sweep."""
+    import torch
+    from paper_2502_06073_b200 import binding as B
+    from paper_2502_06073_b200 import workloads as WL
+    torch.cuda.set_device(0)
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    n_sm = torch.cuda.get_device_properties(0).multi_processor_count
+    out = []
+    for k in [int(x) for x in args.sweep.split(",")]:
+        ent = {"log2_n": k}
+        try:
+            w = WL.get(4, log2_n=k)
+            n_md = args.md_steps or (10 if k <= 21 else 3)
+            N = w.n_atoms
+            model = B.Allegro(B.build_weights(w.hp, w.weight_seed), w.hp)
+            vel0 = WL.maxwell_boltzmann(w.mass, w.temperature, w.vel_seed)
+            dev = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a, dtype=dt)).cuda()
+            model.md_init(dev(w.pos, np.float64), dev(vel0, np.float64), dev(w.mass, np.float64), dev(w.species, np.int32), w.cell,
+                          w.hp["r_cut"], w.skin)
+            model.md_step(w.dt_fs, 2)
+            torch.cuda.synchronize()
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ev0.record()
+            for _ in range(args.steps):
+                model.md_step(w.dt_fs, n_md)
+            ev1.record(); torch.cuda.synchronize()
+            ms = ev0.elapsed_time(ev1) / (args.steps * n_md)
+            st = model.get_stats()
+            model.profile(True); model.md_step(w.dt_fs, 2); prof = model.get_profile(); model.profile(False)
+            for v in prof.values():
+                v["ms"] /= 2.0; v["work"] /= 2.0
+            roof = roofline_for(prof, st, None, peaks, n_sm, N, ms)
+            free_b, total_b = torch.cuda.mem_get_info()
+            ent.update({"n_atoms": N, "active_edges": st["active_edges"], "list_edges": st["list_edges"], "chunks": st["chunks"],
+                        "ms_per_md_step": ms, "atom_steps_per_s": N / (ms * 1e-3), "per_step_roofline_frac": roof["per_step"]["frac"],
+                        "t_roof_ms": roof["per_step"]["t_roof_ms"], "device_mem_used_gb": (total_b - free_b) / 1e9})
+            del model
+            torch.cuda.empty_cache()
+        except Exception as e:   # out of memory (host or device) ends the sweep
+            ent["error"] = str(e)[:200]
+            out.append(ent)
+            break
+        out.append(ent)
+    print(json.dumps({"metric": METRIC, "unit": UNIT, "sweep": "BASELINE.json configs[4] (config-1 network, tiled SiO2-like boxes)",
+                      "n_gpus": 1, "data": "synthetic", "entries": out}))
 
 
 def main():
     args = parse()
     if args.impl == "reference":
         run_reference(args)
+    elif args.sweep:
+        run_sweep(args)
     else:
         run_ours(args)
 

@@ -560,7 +560,7 @@ bool launch_gemm_f16s(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t s
   }
   const int64_t tiles = ((m_cap * a.m_mul + fa.rpt - 1) / fa.rpt) * fa.n_nt;
   const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(tiles, m->num_sms));
-  prof_begin(m, st, KC_GEMM, 2.0 * a.N * K * a.m_mul);
+  prof_begin(m, st, KC_GEMM16, 2.0 * a.N * K * a.m_mul);
   k_gemm_f16s<<<grid, F_T, F_SMEM, st>>>(fa, t0, t1, tc, tc2);
   prof_end(m, st);
   m->launches += 1;

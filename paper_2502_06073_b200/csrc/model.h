@@ -70,7 +70,7 @@ struct Workspace {       // per-chunk activations, sized for cap_edges active ed
 };
 
 // optional per-kernel-class timing with CUDA events on the launching stream (allegro_profile)
-enum { KC_GEMM = 0, KC_TP_FWD, KC_TP_BWD, KC_GAMMA, KC_GAMMABAR, KC_ACTIVE, KC_EDGE_MISC, KC_NEIGHBOR, KC_MD, KC_GATHER, KC_COUNT };
+enum { KC_GEMM = 0, KC_TP_FWD, KC_TP_BWD, KC_GAMMA, KC_GAMMABAR, KC_ACTIVE, KC_EDGE_MISC, KC_NEIGHBOR, KC_MD, KC_GATHER, KC_GEMM16, KC_COUNT };
 struct Prof {
   bool on = false;
   std::vector<cudaEvent_t> ev;      // pairs

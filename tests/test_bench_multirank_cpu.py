@@ -41,9 +41,22 @@ def test_max_over_ranks_and_whole_job_value_gloo_world2():
 def test_roofline_object_shape():
     sys.path.insert(0, ROOT)
     import bench
-    prof = {"gemm": dict(ms=2.0, launches=10, work=1.0e5), "tp_fwd": dict(ms=0.5, launches=2, work=3.0e4), "md": dict(ms=0.1, launches=4, work=0.0)}
-    roof = bench.roofline_for(prof, {"active_edges": 100000}, {"sm_max_mhz": 1965.0}, {"bf16_tflops_sustained": 1379.3}, 148)
-    assert roof["bound"] == "tensor" and roof["unit"] == "TFLOP/s" and roof["kernel"] == "k_gemm_chain"
+    prof = {"gemm_f16s": dict(ms=2.0, launches=10, work=1.0e5), "gemm": dict(ms=0.2, launches=2, work=1.0e4),
+            "tp_fwd": dict(ms=0.5, launches=2, work=3.0e4), "md": dict(ms=0.1, launches=4, work=0.0)}
+    stats = {"active_edges": 100000, "list_edges": 130000, "chunks": 1}
+    peaks = {"bf16_tflops": 1668.6, "bf16_tflops_sustained": 1361.0, "hbm_gbs": 6548.8}
+    roof = bench.roofline_for(prof, stats, {"sm_max_mhz": 1965.0, "sm_mhz": 1965.0}, peaks, 148, 4096, 3.0)
+    assert roof["bound"] == "tensor" and roof["unit"] == "TFLOP/s" and roof["kernel"] == "k_gemm_f16s"
     assert abs(roof["achieved"] - 1.0e5 * 1e5 / 2e-3 / 1e12) < 1e-9
+    assert abs(roof["peak"] - 1668.6 / 3.0) < 1e-9                       # burst peak: the clock stayed at max; 3 fp16 passes
     assert abs(roof["frac"] - roof["achieved"] / roof["peak"]) < 1e-12
     assert abs(sum(roof["shares"].values()) - 1.0) < 1e-3
+    ps = roof["per_step"]
+    t_tensor = (1.0e4 * 1e5 / (1668.6 * (1.1 / 2.25) / 3 * 1e12) + 1.0e5 * 1e5 / (1668.6 / 3 * 1e12)) * 1e3
+    assert abs(ps["t_tensor_ms"] - t_tensor) < 1e-9
+    assert abs(ps["t_alu_ms"] - 3.0e4 * 1e5 / (148 * 128 * 2 * 1965e6) * 1e3) < 1e-9
+    assert abs(ps["t_hbm_ms"] - (148.0 * 4096 + 8 * 130000) / 6548.8e9 * 1e3) < 1e-12
+    assert ps["t_roof_ms"] == max(ps["t_tensor_ms"], ps["t_alu_ms"], ps["t_hbm_ms"]) and abs(ps["frac"] - ps["t_roof_ms"] / 3.0) < 1e-12
+    # below-max clocks select the sustained peak
+    roof2 = bench.roofline_for(prof, stats, {"sm_max_mhz": 1965.0, "sm_mhz": 1500.0}, peaks, 148, 4096, 3.0)
+    assert abs(roof2["peak"] - 1361.0 / 3.0) < 1e-9
