@@ -133,9 +133,10 @@ int allegro_get_stats(void* h, int64_t* stats);
 /* Per-kernel-class timing for bench.py's roofline line.  allegro_profile(h, 1) resets the counters and makes
  * every launch of the following calls bracketed by CUDA events on the launching stream; allegro_profile(h, 0)
  * stops it.  allegro_get_profile synchronises and returns, per class k (0 gemm, 1 tp_fwd, 2 tp_bwd, 3 gamma,
- * 4 gammabar, 5 active_edges, 6 edge_misc, 7 neighbor, 8 md, 9 force_gather, 10 gemm_f16s; class 0 = the 3xTF32 kernels of
- * gemm_tc.cu, class 10 = the split-fp16 kernel of gemm_f16s.cu): ms[k] total device time, launches[k], work[k] = algorithmic
- * flop per active edge summed over the class's launches (classes 0-2 and 10, else 0).
+ * 4 gammabar, 5 active_edges, 6 edge_misc, 7 neighbor, 8 md, 9 force_gather, 10 gemm_f16s, 11 tp_mix; class 0 = the 3xTF32 kernels of
+ * gemm_tc.cu, class 10 = the split-fp16 kernel of gemm_f16s.cu, class 11 carries only work: the channel-mixing flop that the
+ * few-channel tensor-product kernels run on mma.sync inside classes 1-2): ms[k] total device time, launches[k], work[k] =
+ * algorithmic flop per active edge summed over the class's launches (classes 0-2, 10, 11, else 0).
  * HOST arrays of max_classes entries; returns the number of classes.  Never enabled inside a timed throughput run. */
 int allegro_profile(void* h, int enable);
 int allegro_get_profile(void* h, double* ms, int64_t* launches, double* work, int max_classes);

@@ -319,22 +319,24 @@ def _cell_lengths(cell):
     return np.diag(cell).copy()
 
 
-def neighbors_bruteforce(pos, cell, radius):
+def neighbors_bruteforce(pos, cell, radius, rows=None):
     """All ordered (i, j, s) with |r_j + s.cell - r_i| < radius, (i,j,s) != (i,i,0): O(N^2 * 27).
 
     A16: d^2 = dx^2+dy^2+dz^2 in fp64 with dx = (x_j - x_i) + s_x L_x, compared as d^2 < radius^2.
     A17: requires radius <= min(L); the three images nearest to the rounded minimum image are tried
     per axis, which then covers every image inside the sphere.  Returns CSR (rowptr int64, col int32,
-    shift int32 [E,3]) with each row sorted by (j, sx, sy, sz)."""
+    shift int32 [E,3]) with each row sorted by (j, sx, sy, sz).  ``rows``: only these centre atoms (CSR over
+    them, in the given order) - the same loop body, used to sample rows of systems too large for N^2."""
     pos = np.asarray(pos, dtype=np.float64)
     Ld = _cell_lengths(cell)
     if radius > Ld.min():
         raise ValueError("radius exceeds the smallest box length")
     N = pos.shape[0]
     R2 = radius * radius
-    rows_j, rows_s, counts = [], [], np.zeros(N, np.int64)
+    centres = np.arange(N) if rows is None else np.asarray(rows)
+    rows_j, rows_s, counts = [], [], np.zeros(centres.size, np.int64)
     trip = np.array([(a, b, c) for a in (-1, 0, 1) for b in (-1, 0, 1) for c in (-1, 0, 1)], dtype=np.int64)
-    for i in range(N):
+    for q, i in enumerate(centres):
         d0 = pos - pos[i]                                   # x_j - x_i
         n0 = -np.round(d0 / Ld).astype(np.int64)            # image bringing j closest to i
         s = n0[:, None, :] + trip[None, :, :]               # [N,27,3]
@@ -345,10 +347,10 @@ def neighbors_bruteforce(pos, cell, radius):
         jj, tt = np.nonzero(ok)
         ss = s[jj, tt]
         order = np.lexsort((ss[:, 2], ss[:, 1], ss[:, 0], jj))
-        rows_j.append(jj[order]); rows_s.append(ss[order]); counts[i] = jj.size
+        rows_j.append(jj[order]); rows_s.append(ss[order]); counts[q] = jj.size
     rowptr = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
-    col = np.concatenate(rows_j).astype(np.int32) if N else np.zeros(0, np.int32)
-    shift = np.concatenate(rows_s).astype(np.int32) if N else np.zeros((0, 3), np.int32)
+    col = np.concatenate(rows_j).astype(np.int32) if centres.size else np.zeros(0, np.int32)
+    shift = np.concatenate(rows_s).astype(np.int32) if centres.size else np.zeros((0, 3), np.int32)
     return rowptr, col, shift
 
 

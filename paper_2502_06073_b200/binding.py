@@ -29,7 +29,7 @@ EXPORTS = ["allegro_weight_layout", "allegro_create", "allegro_destroy", "allegr
            "allegro_debug_coupling", "allegro_debug_num_paths", "allegro_debug_set_precision", "allegro_debug_gemm",
            "allegro_last_error"]
 PROFILE_CLASSES = ["gemm", "tp_fwd", "tp_bwd", "gamma", "gammabar", "active_edges", "edge_misc", "neighbor", "md",
-                   "force_gather", "gemm_f16s"]
+                   "force_gather", "gemm_f16s", "tp_mix"]
 
 
 class HParams(C.Structure):

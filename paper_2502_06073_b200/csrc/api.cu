@@ -145,10 +145,6 @@ int allegro_create(const float* weights_host, size_t n_weights, const allegro_hp
     delete m; return ALLEGRO_ERR_CUDA;
   }
   cudaGetDevice(&m->device);
-  { const char* g = std::getenv("ALLEGRO_GEMM"); m->use_tc = !(g && std::string(g) == "fp32"); }
-  { const char* g = std::getenv("ALLEGRO_GRAPH"); m->use_graph = !(g && std::string(g) == "0"); }
-  { const char* g = std::getenv("ALLEGRO_CHAIN"); m->use_chain = !(g && std::string(g) == "0"); }
-  { const char* g = std::getenv("ALLEGRO_TP"); m->use_tp3 = !(g && std::string(g) == "generic"); }
   m->use_big = m->use_tc && m->use_tp3 && (hp->n_channels == 64 || hp->n_channels == 128 || hp->n_channels == 256);
   cudaDeviceGetAttribute(&m->num_sms, cudaDevAttrMultiProcessorCount, m->device);
   auto fail = [&](int rc, const std::string& msg) { g_create_err = msg; allegro_destroy(m); return rc; };

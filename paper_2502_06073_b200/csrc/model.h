@@ -70,7 +70,7 @@ struct Workspace {       // per-chunk activations, sized for cap_edges active ed
 };
 
 // optional per-kernel-class timing with CUDA events on the launching stream (allegro_profile)
-enum { KC_GEMM = 0, KC_TP_FWD, KC_TP_BWD, KC_GAMMA, KC_GAMMABAR, KC_ACTIVE, KC_EDGE_MISC, KC_NEIGHBOR, KC_MD, KC_GATHER, KC_GEMM16, KC_COUNT };
+enum { KC_GEMM = 0, KC_TP_FWD, KC_TP_BWD, KC_GAMMA, KC_GAMMABAR, KC_ACTIVE, KC_EDGE_MISC, KC_NEIGHBOR, KC_MD, KC_GATHER, KC_GEMM16, KC_TP_MIX, KC_COUNT };
 struct Prof {
   bool on = false;
   std::vector<cudaEvent_t> ev;      // pairs
@@ -87,10 +87,10 @@ struct Model {
   std::string err;
   int device = 0;
   int num_sms = 148;
-  bool use_tc = true;              // dense linears on tcgen05 (3xTF32); ALLEGRO_GEMM=fp32 selects the FP32-pipe kernel
-  bool use_chain = true;           // MLP chains in one kernel (gemm_tc.cu k_gemm_chain); ALLEGRO_CHAIN=0 launches stage by stage
+  bool use_tc = true;              // dense linears on tcgen05
+  bool use_chain = true;           // MLP chains in one kernel (gemm_tc.cu k_gemm_chain) where the widths fit
   bool use_big = false;            // many-channel tensor product: T buffers + tcgen05 channel mixing (tp_big.cuh)
-  bool use_tp3 = true;             // few-channel tensor-product kernels (tp3.cuh); ALLEGRO_TP=generic selects tp.cuh
+  bool use_tp3 = true;             // few-channel tensor-product kernels (tp3.cuh) where the channel count is 8, 16 or 32, else tp.cuh
   float* d_w = nullptr;            // weight blob
   float* d_weff = nullptr;         // collapsed edge-energy chain W_last...W_1 -> [D]
   std::vector<CgDev> cg;           // per layer

@@ -115,15 +115,17 @@ int ws_prepare(Model* m, int64_t cap_edges, int64_t cap_atoms) {
   return 0;
 }
 
-// algorithmic flop per active edge of one layer's tensor product (+ channel mixing): 3 flop per coupling nonzero
-// and channel, 2 n^2 (2l+1) per path through W_lin; the backward has two coupling products.
-static double tp_work(const Plan& P, int L, bool backward) {
+// algorithmic flop per active edge of one layer's tensor product on the FP32 pipe: 3 flop per coupling nonzero and channel
+// (the backward has two coupling products); mix = the channel-mixing flop 2 n^2 (2l+1) per path through W_lin, which run on
+// the tensor cores (mma.sync inside k_tp_*3, or the GEMM kernels for many channels, where the GEMM class counts them).
+static double tp_work(const Plan& P, int L, bool backward, double* mix) {
   const Layer& ly = P.layers[L - 1];
   const double n = P.hp.n_channels;
   double f = 0;
+  *mix = 0;
   for (const Path& p : ly.paths) {
     f += (backward ? 6.0 : 3.0) * n * (p.cg_end - p.cg_begin);
-    if (L < P.hp.n_layers) f += 2.0 * n * n * (2 * ly.out_irreps[p.iro].l + 1);
+    if (L < P.hp.n_layers) *mix += 2.0 * n * n * (2 * ly.out_irreps[p.iro].l + 1);
   }
   return f;
 }
@@ -250,7 +252,9 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
     io.s = ws.s[L - 1]; io.vout = (L < NL) ? ws.V[L - 1] : nullptr;
     {
       dim3 grid((unsigned)((m_cap + TE - 1) / TE), (unsigned)(tp.has_lin ? tp.n_out : 1));
-      prof_begin(m, st, KC_TP_FWD, tp_work(P, L, false));
+      double mixf = 0;
+      prof_begin(m, st, KC_TP_FWD, tp_work(P, L, false, &mixf));
+      if (m->prof.on && !(m->use_big && tpbig_supported(tp))) m->prof.work[KC_TP_MIX] += mixf;
       if (m->use_big && tpbig_supported(tp)) {
         // many channels: tensor product to per-irrep T buffers, channel mixing as tcgen05 GEMMs written straight into V^L
         TpBig big{};
@@ -373,7 +377,9 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
       io.sbar = ws.sb; io.vbar = (L < NL) ? ws.vb[vcur] : nullptr; io.vbar_prev = ws.vb[vcur ^ 1]; io.ge = ws.ge;
       io.wbar_init = ws.wb; io.ldwb = 2 * nsc; io.ybar = ws.yb;   // layer 1: B8 applied inside the kernel
       size_t smem = smem_of(TE, PC);
-      prof_begin(m, st, KC_TP_BWD, tp_work(P, L, true));
+      double mixb = 0;
+      prof_begin(m, st, KC_TP_BWD, tp_work(P, L, true, &mixb));
+      if (m->prof.on && !(m->use_big && tpbig_supported(tp))) m->prof.work[KC_TP_MIX] += mixb;
       if (m->use_big && tpbig_supported(tp)) {
         TpBig big{};
         size_t off = 0;

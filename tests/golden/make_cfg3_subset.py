@@ -1,0 +1,51 @@
+"""Writes tests/golden/cfg3_subset.npz: fp64 oracle results on a seeded subset of BASELINE.json configs[3] (262,144 atoms,
+FM-sized network), for tests/test_gpu_parity_large.py.  Calls only oracle/ and the seeded generators of workloads.py; nothing
+here comes from the CUDA path.  The numpy oracle needs ~1.1 s per centre atom of this network on 8 cores, so the subset is
+16 force targets with their closure (every atom within r_c of a target: ~1,200 centre atoms, all of which also give a
+per-atom energy) — SURVEY.md 8d asks for 128 targets / 1,024 E_i; the E_i count is met, the force targets are what fits in
+~25 minutes of host time.  Also stored: the list rows (col, shift) at r_c + skin of 64 sampled atoms for the bit-exact
+neighbour gate.  Run:  python tests/golden/make_cfg3_subset.py"""
+import os
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+sys.path.insert(0, ROOT)
+from oracle import allegro_oracle as O                      # noqa: E402
+from paper_2502_06073_b200 import workloads as WL           # noqa: E402
+
+N_TARGETS, N_LIST_ROWS, SEED = 16, 64, 13
+
+
+def main():
+    w = WL.get(3)
+    rc, skin = w.hp["r_cut"], w.skin
+    t0 = time.time()
+    rp, col, sh = O.neighbors_binned(w.pos, w.cell, rc)
+    rng = np.random.default_rng(SEED)
+    T = np.sort(rng.choice(w.n_atoms, N_TARGETS, replace=False))
+    closure = set(T.tolist())
+    for i in T:
+        closure.update(col[rp[i]:rp[i + 1]].tolist())
+    cen = np.array(sorted(closure))
+    print("targets", T.size, "centres", cen.size, "edges", int(sum(rp[a + 1] - rp[a] for a in cen)), flush=True)
+    model = O.AllegroOracle(w.hp, WL.make_weights(O.weight_layout(w.hp), w.hp, w.weight_seed))
+    E, F, Ea = model.energy_forces(w.pos, w.species, w.cell, (rp, col, sh), centres=cen, max_edges_per_chunk=20000)
+    print("oracle done in %.0f s" % (time.time() - t0), flush=True)
+    # list rows at the list radius for the bit-exact neighbour gate
+    rpl, coll, shl = O.neighbors_binned(w.pos, w.cell, rc + skin)
+    rows = np.sort(np.concatenate([T, rng.choice(w.n_atoms, N_LIST_ROWS - N_TARGETS, replace=False)]))
+    row_ptr = np.concatenate([[0], np.cumsum([rpl[a + 1] - rpl[a] for a in rows])]).astype(np.int64)
+    row_col = np.concatenate([coll[rpl[a]:rpl[a + 1]] for a in rows]).astype(np.int32)
+    row_sh = np.concatenate([shl[rpl[a]:rpl[a + 1]] for a in rows]).astype(np.int8)
+    out = os.path.join(os.path.dirname(os.path.abspath(__file__)), "cfg3_subset.npz")
+    np.savez_compressed(out, targets=T, centres=cen, E_atom=Ea[cen], F_targets=F[T], n_active_edges=np.int64(rp[-1]),
+                        n_list_edges=np.int64(rpl[-1]), list_rows=rows, list_rowptr=row_ptr, list_col=row_col, list_shift=row_sh,
+                        list_row_len_all_sum=np.int64(rpl[-1]), seed=np.int64(SEED))
+    print("wrote", out, "in %.0f s" % (time.time() - t0))
+
+
+if __name__ == "__main__":
+    main()

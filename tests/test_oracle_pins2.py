@@ -42,6 +42,11 @@ def test_binned_equals_bruteforce_three_or_more_cells(box):
     for x, y in zip(a, b):
         assert np.array_equal(x, y)
     assert a[0][-1] > 4000
+    # the row-sampled form of the brute-force search is the same loop restricted to those centres
+    rows = np.array([7, 0, 399, 123])
+    rp, col, sh = O.neighbors_bruteforce(pos, cell, radius, rows=rows)
+    for q, i in enumerate(rows):
+        assert np.array_equal(col[rp[q]:rp[q + 1]], b[1][b[0][i]:b[0][i + 1]]) and np.array_equal(sh[rp[q]:rp[q + 1]], b[2][b[0][i]:b[0][i + 1]])
 
 
 # ---------------------------------------------------------------- subset and chunked evaluation
