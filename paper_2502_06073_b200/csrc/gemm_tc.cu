@@ -50,7 +50,8 @@ __global__ void k_pack_w(const float* __restrict__ W, int ldw, int wtrans, int N
 }
 
 // smem per stage: A_hi | A_lo (128 x 16 fp32 each = 8 KB) | B_hi | B_lo (Nt x 16 fp32 each)
-__global__ void __launch_bounds__(TC_T + 32) k_gemm_tc(GemmArgs a, const float* __restrict__ Bp, int Npad, int Kpad, int tmem_cols, int vec_ok) {
+__global__ void __launch_bounds__(TC_T + 32) k_gemm_tc(GemmArgs a, const float* __restrict__ Bp, int Npad, int Kpad, int tmem_cols, int vec_ok,
+                                                       int passes) {
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t mbar_mma[2];
   __shared__ __align__(8) uint64_t mbar_b[2];
@@ -105,9 +106,10 @@ __global__ void __launch_bounds__(TC_T + 32) k_gemm_tc(GemmArgs a, const float* 
           const uint32_t koff = ks * 256;                              // two 128-byte k-chunks per K=8 step
           const uint64_t dAh = umma_desc(sa_hi + koff, 128, sbo), dAl = umma_desc(sa_lo + koff, 128, sbo);
           const uint64_t dBh = umma_desc(sb_hi + koff, 128, sbo), dBl = umma_desc(sb_lo + koff, 128, sbo);
-          umma_tf32(tmem_d, dAl, dBh, idesc, (c > 0 || ks > 0) ? 1u : 0u);   // small terms first
-          umma_tf32(tmem_d, dAh, dBl, idesc, 1u);
-          umma_tf32(tmem_d, dAh, dBh, idesc, 1u);
+          const uint32_t acc = (c > 0 || ks > 0) ? 1u : 0u;
+          if (passes >= 2) umma_tf32(tmem_d, dAl, dBh, idesc, acc);   // small terms first
+          if (passes >= 3) umma_tf32(tmem_d, dAh, dBl, idesc, 1u);
+          umma_tf32(tmem_d, dAh, dBh, idesc, passes >= 2 ? 1u : acc);
         }
         umma_commit(&mbar_mma[b]);
       }
@@ -291,7 +293,7 @@ void launch_gemm_tc(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st)
   if (a.epi == EPI_SPLIT_RES) vec_ok = vec_ok && (a.split % 4 == 0);
   dim3 grid((unsigned)((m_cap + TC_M - 1) / TC_M), (unsigned)((Npad + TC_NMAX - 1) / TC_NMAX));
   prof_begin(m, st, KC_GEMM, 2.0 * a.N * K * a.m_mul);
-  k_gemm_tc<<<grid, TC_T + 32, smem, st>>>(a, Bp, Npad, Kpad, tmem_cols, vec_ok);
+  k_gemm_tc<<<grid, TC_T + 32, smem, st>>>(a, Bp, Npad, Kpad, tmem_cols, vec_ok, m->f16_passes);
   prof_end(m, st);
   m->launches += 1;
 }
@@ -313,6 +315,7 @@ constexpr int CH_MAX = 4, CH_NB = 3, CH_KMAX = 128, CH_NMAX = 128, CH_T = TC_T +
 
 struct ChainArgs {
   int n;
+  int passes;                    // 3 = hi*hi + hi*lo + lo*hi (default); 2 / 1 only for the precision study (R4)
   GemmArgs st[CH_MAX];
   const float* Bp[CH_MAX];
   const float* WgT[CH_MAX];      // EPI_GATHER2: species columns of W transposed, [2S][N]
@@ -398,9 +401,10 @@ __global__ void __launch_bounds__(CH_T, 2) k_gemm_chain(const __grid_constant__ 
             const uint32_t koff = ks * 256;
             const uint64_t dAh = umma_desc(sa_hi + koff, 128, sbo), dAl = umma_desc(sa_lo + koff, 128, sbo);
             const uint64_t dBh = umma_desc(sb_hi + koff, 128, sbo), dBl = umma_desc(sb_lo + koff, 128, sbo);
-            umma_tf32(tmem_dd, dAl, dBh, idesc, (c > 0 || ks > 0) ? 1u : 0u);
-            umma_tf32(tmem_dd, dAh, dBl, idesc, 1u);
-            umma_tf32(tmem_dd, dAh, dBh, idesc, 1u);
+            const uint32_t acc = (c > 0 || ks > 0) ? 1u : 0u;
+            if (ca.passes >= 2) umma_tf32(tmem_dd, dAl, dBh, idesc, acc);
+            if (ca.passes >= 3) umma_tf32(tmem_dd, dAh, dBl, idesc, 1u);
+            umma_tf32(tmem_dd, dAh, dBh, idesc, ca.passes >= 2 ? 1u : acc);
           }
           umma_commit(&mbar_s[slot]);
         }
@@ -670,6 +674,7 @@ bool launch_gemm_chain(Model* m, const GemmArgs* stages, int n_stages, int64_t m
   if (!m->use_tc || !m->use_chain || n_stages < 1 || n_stages > CH_MAX || m_cap <= 0) return false;
   ChainArgs ca{};
   ca.n = n_stages;
+  ca.passes = m->f16_passes;
   auto al = [](const void* p) { return ((uintptr_t)p & 15) == 0; };
   double work = 0;
   int nmax = 16;

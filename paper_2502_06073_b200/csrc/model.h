@@ -97,7 +97,7 @@ struct Model {
   std::vector<int> tp_sig;         // per layer: index of the generated coupling code (tp_gen.cuh)
   std::map<std::array<int64_t, 5>, float*> packed_w;   // tcgen05 B operands: hi/lo split, canonical UMMA layout (gemm_tc.cu)
   std::map<std::array<int64_t, 6>, TMapStore> tmaps;   // TMA tensor maps of the A operands, by (pointer, K, ld, rows) (gemm_f16s.cu)
-  int f16_passes = 3;              // split-fp16 products per element: 3 (default), 2 or 1 only for the precision study (R4)
+  int f16_passes = 3;              // tensor-core passes per product in every GEMM kernel: 3 (default); 2 or 1 only for the precision study (R4)
   int64_t f16_rows_cap = 0;        // rows every edge-sized workspace array holds (bounds the tensor maps)
   std::vector<float> c_old, c_new; // host copies
   NeighborList nl;
