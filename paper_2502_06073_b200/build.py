@@ -18,6 +18,8 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr", "-Xptxas", "-v" if os.environ.get("ALLEGRO_PTXAS_V") else "-O3"]
 if os.environ.get("ALLEGRO_F16S_TRACE"):   # developer build: gemm_f16s.cu prints the per-tile timeline of CTA 0 after every launch
     NVCC_FLAGS.append("-DF16S_TRACE")
+if os.environ.get("ALLEGRO_F16S_DBGWAIT"):   # developer build: barrier waits time out and report their source line instead of trapping
+    NVCC_FLAGS.append("-DF16S_DBGWAIT")
 
 
 def _stale() -> bool:

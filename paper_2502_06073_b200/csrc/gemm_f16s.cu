@@ -52,8 +52,8 @@ constexpr uint32_t F_CVT_BYTES = F_M * F_KS * 2;                        // one o
 constexpr uint32_t F_BMAX_BYTES = F_NT * F_KS * 2;                      // one of B_hi / B_lo at 256 columns
 constexpr uint32_t F_OFF_CVT = F_RAW_BYTES, F_OFF_B = F_RAW_BYTES + 2 * F_CVT_BYTES;
 constexpr uint32_t F_STAGE_BYTES = F_OFF_B + 2 * F_BMAX_BYTES;          // 64 KB
-constexpr uint32_t F_OUT_BYTES = F_M * 16 * 4;                          // one 128 x 16 fp32 epilogue tile; two per epilogue group
-constexpr size_t F_SMEM = (size_t)F_S * F_STAGE_BYTES + 4 * F_OUT_BYTES + 1024;
+constexpr uint32_t F_OUT_BYTES = F_M * 32 * 4;                          // one 128 x 32 fp32 output tile per epilogue group
+constexpr size_t F_SMEM = (size_t)F_S * F_STAGE_BYTES + 2 * F_OUT_BYTES + 1024;
 constexpr float F_LO_SCALE = 2048.0f, F_LO_INV = 1.0f / 2048.0f;
 
 struct FArgs {
@@ -65,7 +65,6 @@ struct FArgs {
   int passes;               // 3 = full split, 2 = activations split only, 1 = plain fp16 (precision study)
   int rpt;                  // rows per tile: 128, or d3 * (128 / d3) when rows are (edge, m) pairs of a mapped operand
   int a_d3, c_d3;           // > 0: A0 / C is the 3-D mapped tensor
-  unsigned long long* trace; // F16S_TRACE builds: per-tile clock64 stamps of CTA 0
 };
 
 // bounded wait: a protocol error ends in a trap (sticky CUDA error) instead of a hung GPU
@@ -143,11 +142,10 @@ __global__ void k_pack_w16(const float* __restrict__ W, int ldw, int wtrans, int
 
 __global__ void __launch_bounds__(F_T, 1) k_gemm_f16s(const __grid_constant__ FArgs fa, const __grid_constant__ CUtensorMap tmA0,
                                                        const __grid_constant__ CUtensorMap tmA1, const __grid_constant__ CUtensorMap tmC,
-                                                       const __grid_constant__ CUtensorMap tmC2, const __grid_constant__ CUtensorMap tmX) {
+                                                       const __grid_constant__ CUtensorMap tmC2) {
   extern __shared__ uint8_t smem_dyn[];
   __shared__ __align__(8) uint64_t raw_full[F_S], raw_empty[F_S], cvt_full[F_S], b_full[F_S], mma_done[F_S];
   __shared__ __align__(8) uint64_t acc_full, acc_empty;
-  __shared__ __align__(8) uint64_t x_full[2][2];           // auxiliary rows landed in tile [group][buffer]
   __shared__ uint32_t tmem_base_s;
   const GemmArgs& a = fa.a;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -170,7 +168,6 @@ __global__ void __launch_bounds__(F_T, 1) k_gemm_f16s(const __grid_constant__ FA
       mbar_init(&b_full[s], 1); mbar_init(&mma_done[s], 1);
     }
     mbar_init(&acc_full, 1); mbar_init(&acc_empty, F_EPI);
-    mbar_init(&x_full[0][0], 1); mbar_init(&x_full[0][1], 1); mbar_init(&x_full[1][0], 1); mbar_init(&x_full[1][1], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -228,27 +225,12 @@ __global__ void __launch_bounds__(F_T, 1) k_gemm_f16s(const __grid_constant__ FA
         const int Nt = min(fa.Npad - nt * F_NT, F_NT);
         // D fp32 (bit 4), A/B fp16 (0 at bits 7 and 10), both K-major, N >> 3 at bit 17, M >> 4 at bit 24
         const uint32_t idesc = (1u << 4) | ((uint32_t)(Nt >> 3) << 17) | ((uint32_t)(F_M >> 4) << 24);
-#ifdef F16S_TRACE
-        const long long t_a = clock64();
-#endif
         mbar_wait_b(&acc_empty, (titer & 1) ^ 1);
-#ifdef F16S_TRACE
-        const long long t_b = clock64();
-        long long w_cvt = 0, w_b = 0;
-#endif
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         for (int ks = 0; ks < nk; ++ks, ++it) {
           const uint32_t slot = it % F_S, ph = (it / F_S) & 1;
-#ifdef F16S_TRACE
-          const long long t0 = clock64();
-          mbar_wait_b(&cvt_full[slot], ph);
-          const long long t1 = clock64();
-          mbar_wait_b(&b_full[slot], ph);
-          w_cvt += t1 - t0; w_b += clock64() - t1;
-#else
           mbar_wait_b(&cvt_full[slot], ph);
           mbar_wait_b(&b_full[slot], ph);
-#endif
           asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
           const uint32_t sbase = smem_u32(smem + (size_t)slot * F_STAGE_BYTES);
           const uint32_t sa_hi = sbase + F_OFF_CVT, sa_lo = sa_hi + F_CVT_BYTES;
@@ -266,9 +248,6 @@ __global__ void __launch_bounds__(F_T, 1) k_gemm_f16s(const __grid_constant__ FA
           umma_commit(&mma_done[slot]);
         }
         umma_commit(&acc_full);
-#ifdef F16S_TRACE
-        if (fa.trace && blockIdx.x == 0 && titer < 16) { unsigned long long* q = fa.trace + titer * 16; q[0] = t_a; q[1] = t_b; q[2] = clock64(); q[3] = w_cvt; q[4] = w_b; }
-#endif
       }
     }
   } else if (warp < F_W_EPI0) {
@@ -291,19 +270,8 @@ __global__ void __launch_bounds__(F_T, 1) k_gemm_f16s(const __grid_constant__ FA
       for (int ks = 0; ks < nk; ++ks, ++it) {
         const uint32_t slot = it % F_S, ph = (it / F_S) & 1;
         uint8_t* st = smem + (size_t)slot * F_STAGE_BYTES;
-#ifdef F16S_TRACE
-        const long long tc0 = clock64();
-        mbar_wait_b(&raw_full[slot], ph);
-        const long long tc1 = clock64();
-        mbar_wait_b(&mma_done[slot], ph ^ 1);
-        if (fa.trace && blockIdx.x == 0 && cw == 0 && lane == 0 && it < 16 * (uint32_t)nk) {
-          unsigned long long* q = fa.trace + (it / nk) * 16;
-          q[8] += tc1 - tc0; q[9] += clock64() - tc1;
-        }
-#else
         mbar_wait_b(&raw_full[slot], ph);
         mbar_wait_b(&mma_done[slot], ph ^ 1);
-#endif
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
           const int r = 16 * cw + 8 * i + r7;
@@ -330,29 +298,20 @@ __global__ void __launch_bounds__(F_T, 1) k_gemm_f16s(const __grid_constant__ FA
       }
     }
   } else {
-    // ---- epilogue: two groups of four warps (TMEM lane quadrant = warp % 4).  A group works through its items (16-column step,
-    // pass) with two 128 x 16 tiles in shared memory (SWIZZLE_64B, conflict-free one row per lane): the auxiliary rows of item
-    // i + 1 (residual input, saved pre-activation, accumulation target) are TMA-loaded into one tile while item i is computed
-    // IN PLACE in the other (a lane overwrites exactly the chunks it read) and TMA-stored.  The auxiliary tile of the whole
-    // output tile is prefetched into L2 while the tensor pipe still works on it, so those loads do not wait for HBM.
+    // ---- epilogue: two groups of four warps (TMEM lane quadrant = warp % 4); a group takes alternate 32-column steps, builds
+    // the 128 x 32 output tile in shared memory (row per lane, 16-byte chunks XOR-swizzled like the tensor map) and TMA-stores it.
     const int ew = warp - F_W_EPI0;
     const int quad = warp & 3, grp = ew >> 2;
     const int erow = quad * 32 + lane;
     const uint32_t lane_addr = (uint32_t)(quad * 32) << 16;
-    uint8_t* obuf0 = out_tiles + (size_t)grp * 2 * F_OUT_BYTES;
-    const int sw = (erow >> 1) & 3;                           // SWIZZLE_64B: 16-byte chunk index ^= (row / 2) % 4
-    const bool leader = (quad == 0 && lane == 0);            // issues the loads and stores of its group
+    uint8_t* obuf = out_tiles + (size_t)grp * F_OUT_BYTES;
+    uint8_t* orow = obuf + erow * 128;
+    const int sw = erow & 7;
+    const bool leader = (quad == 0 && lane == 0);            // issues the stores of its group
     const int bar_id = 1 + grp;
     const int epb_c = fa.c_d3 ? rpt / fa.c_d3 : 0;
     const int npass = (a.epi == EPI_Y_X || a.epi == EPI_RESIDUAL) ? 2 : 1;
-    const bool any_x = a.epi == EPI_RESIDUAL || a.epi == EPI_DSILU || a.epi == EPI_ACCUM || a.epi == EPI_SPLIT_RES;
-    const int xcols = a.epi == EPI_SPLIT_RES ? a.split : a.N;
-    const uint32_t x_bytes = (uint32_t)rpt * 64;
-    uint32_t titer = 0, xuse[2] = {0, 0};
-    // does item (c16, pass) read auxiliary rows, and which
-    auto needs_x = [&](int nb, int pass) {
-      return a.epi == EPI_DSILU || a.epi == EPI_ACCUM || (a.epi == EPI_SPLIT_RES && nb < a.split) || (a.epi == EPI_RESIDUAL && pass == 1);
-    };
+    uint32_t titer = 0;
     for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++titer) {
       const int mt = (int)(tile / fa.n_nt), nt = (int)(tile % fa.n_nt);
       const int col0 = nt * F_NT, Nt = min(fa.Npad - col0, F_NT);
@@ -363,134 +322,110 @@ __global__ void __launch_bounds__(F_T, 1) k_gemm_f16s(const __grid_constant__ FA
         const float* gq = a.geo + row * GEO_W;
         u = gq[4]; zi = __float_as_int(gq[6]); zj = __float_as_int(gq[7]);
       }
+      const float* xrow = ((a.epi == EPI_ACCUM) ? a.C + row * a.ldc : a.aux + row * a.ldaux);
       const float cu = a.c_new * u;
-      const int n16 = (Nt / 16 - grp + 1) / 2;                // 16-column steps of this group: c16 = grp, grp + 2, ...
-      const int n_items = n16 * npass;
-      if (leader && any_x) {
-        // auxiliary rows of this output tile -> L2, in the shadow of the MMA loop
-        for (int c = grp; c * 16 < Nt; c += 2)
-          if (col0 + c * 16 < xcols)
-            asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global [%0, {%1, %2}];" ::"l"(&tmX), "r"(col0 + c * 16), "r"((int)row0) : "memory");
-        // and the rows of the first item into tile 0
-        if (n_items > 0 && needs_x(col0 + grp * 16, 0)) {
-          asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-          asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&x_full[grp][0])), "r"(x_bytes) : "memory");
-          tma_load_2d(obuf0, &tmX, col0 + grp * 16, (int)row0, &x_full[grp][0]);
-        }
-      }
       mbar_wait_b(&acc_full, titer & 1);
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll 1
-      for (int i = 0; i < n_items; ++i) {
-        const int c16 = grp + 2 * (i / npass), pass = i - (i / npass) * npass;
-        const int n0 = c16 * 16, nb = col0 + n0;               // first column of the step inside the tile / in the matrix
-        const int b = i & 1;
-        uint8_t* obuf = obuf0 + (size_t)b * F_OUT_BYTES;
-        uint8_t* orow = obuf + erow * 64;
+      for (int c32 = grp; c32 * 32 < Nt; c32 += 2) {
+        const int nb = col0 + c32 * 32;                          // first global column of this step
         const bool to_c2 = a.epi == EPI_SPLIT_RES && nb >= a.split;
-        const bool use_x = needs_x(nb, pass);
-        // accumulators of this step: both loads in flight before the single wait
-        uint32_t r0[16], r1[16];
-        asm volatile(
-            "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-            : "=r"(r0[0]), "=r"(r0[1]), "=r"(r0[2]), "=r"(r0[3]), "=r"(r0[4]), "=r"(r0[5]), "=r"(r0[6]), "=r"(r0[7]), "=r"(r0[8]), "=r"(r0[9]),
-              "=r"(r0[10]), "=r"(r0[11]), "=r"(r0[12]), "=r"(r0[13]), "=r"(r0[14]), "=r"(r0[15])
-            : "r"(tmem_d0 + lane_addr + (uint32_t)n0));
-        if (passes >= 2)
-          asm volatile(
-              "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-              : "=r"(r1[0]), "=r"(r1[1]), "=r"(r1[2]), "=r"(r1[3]), "=r"(r1[4]), "=r"(r1[5]), "=r"(r1[6]), "=r"(r1[7]), "=r"(r1[8]), "=r"(r1[9]),
-                "=r"(r1[10]), "=r"(r1[11]), "=r"(r1[12]), "=r"(r1[13]), "=r"(r1[14]), "=r"(r1[15])
-              : "r"(tmem_d1 + lane_addr + (uint32_t)n0));
-        if (leader) {
-          // every earlier store of the group has finished reading its tile; then the other tile can take the next item's rows
-          asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-          if (i + 1 < n_items) {
-            const int c16n = grp + 2 * ((i + 1) / npass), passn = (i + 1) - ((i + 1) / npass) * npass;
-            if (needs_x(col0 + c16n * 16, passn)) {
-              asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&x_full[grp][b ^ 1])), "r"(x_bytes) : "memory");
-              tma_load_2d(obuf0 + (size_t)(b ^ 1) * F_OUT_BYTES, &tmX, col0 + c16n * 16, (int)row0, &x_full[grp][b ^ 1]);
+        const int xlim = a.epi == EPI_SPLIT_RES ? a.split : a.N;
+        const bool need_x = a.epi == EPI_DSILU || a.epi == EPI_ACCUM || (a.epi == EPI_SPLIT_RES && !to_c2);
+#pragma unroll 1
+        for (int pass = 0; pass < npass; ++pass) {
+          // the previous store of this group has finished reading the tile
+          if (leader) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+          asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
+#pragma unroll
+          for (int sub = 0; sub < 2; ++sub) {
+            const int n0 = c32 * 32 + sub * 16, ng = col0 + n0;
+            float v[16];
+            tmem_ld16(tmem_d0 + lane_addr + (uint32_t)n0, v);
+            if (passes >= 2) {
+              float w[16];
+              tmem_ld16(tmem_d1 + lane_addr + (uint32_t)n0, w);
+#pragma unroll
+              for (int j = 0; j < 16; ++j) v[j] = fmaf(w[j], F_LO_INV, v[j]);
             }
-          }
-        }
-        asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
-        if (use_x) { mbar_wait_b(&x_full[grp][b], xuse[b] & 1); xuse[b] += 1; }
-        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-        float v[16];
+            float4 x[4];
+            const bool ldx = (need_x || (a.epi == EPI_RESIDUAL && pass == 1)) && row_ok;
 #pragma unroll
-        for (int j = 0; j < 16; ++j) v[j] = passes >= 2 ? fmaf(__uint_as_float(r1[j]), F_LO_INV, __uint_as_float(r0[j])) : __uint_as_float(r0[j]);
-        float4 x[4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) x[j] = use_x ? *reinterpret_cast<const float4*>(orow + ((j ^ sw) << 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
-        float4 o[4];
+            for (int j = 0; j < 4; ++j) {
+              x[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+              if (ldx && ng + 4 * j < xlim) x[j] = *reinterpret_cast<const float4*>(xrow + ng + 4 * j);
+            }
+            float4 o[4];
 #define F_V(j) make_float4(v[4 * (j)], v[4 * (j) + 1], v[4 * (j) + 2], v[4 * (j) + 3])
-        switch (a.epi) {
-          case EPI_GATHER2: {
-            const float* g1p = fa.WgT + (int64_t)zi * a.N;
-            const float* g2p = fa.WgT + (int64_t)(a.S + zj) * a.N;
+            switch (a.epi) {
+              case EPI_GATHER2: {
+                const float* g1p = fa.WgT + (int64_t)zi * a.N;
+                const float* g2p = fa.WgT + (int64_t)(a.S + zj) * a.N;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const int nn = min(nb + 4 * j, a.N - 4);          // padded columns read a valid address; the store clips them
-              const float4 g1 = *reinterpret_cast<const float4*>(g1p + nn);
-              const float4 g2 = *reinterpret_cast<const float4*>(g2p + nn);
-              const float4 t = F_V(j);
-              o[j] = make_float4(t.x + (g1.x + g2.x), t.y + (g1.y + g2.y), t.z + (g1.z + g2.z), t.w + (g1.w + g2.w));
+                for (int j = 0; j < 4; ++j) {
+                  const int nn = min(ng + 4 * j, a.N - 4);        // padded columns read a valid address; the store clips them
+                  const float4 g1 = *reinterpret_cast<const float4*>(g1p + nn);
+                  const float4 g2 = *reinterpret_cast<const float4*>(g2p + nn);
+                  const float4 t = F_V(j);
+                  o[j] = make_float4(t.x + (g1.x + g2.x), t.y + (g1.y + g2.y), t.z + (g1.z + g2.z), t.w + (g1.w + g2.w));
+                }
+              } break;
+              case EPI_Y_X:
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                  const float4 t = F_V(j);
+                  o[j] = pass == 0 ? t : make_float4(u * t.x, u * t.y, u * t.z, u * t.w);
+                }
+                break;
+              case EPI_RESIDUAL:
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                  const float4 t = F_V(j);
+                  o[j] = pass == 0 ? t
+                                   : make_float4(a.c_old * x[j].x + cu * t.x, a.c_old * x[j].y + cu * t.y, a.c_old * x[j].z + cu * t.z,
+                                                 a.c_old * x[j].w + cu * t.w);
+                }
+                break;
+              case EPI_DSILU:
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                  const float4 t = F_V(j);
+                  o[j] = make_float4(t.x * dsilu_f(x[j].x), t.y * dsilu_f(x[j].y), t.z * dsilu_f(x[j].z), t.w * dsilu_f(x[j].w));
+                }
+                break;
+              case EPI_ACCUM:
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                  const float4 t = F_V(j);
+                  o[j] = make_float4(x[j].x + t.x, x[j].y + t.y, x[j].z + t.z, x[j].w + t.w);
+                }
+                break;
+              case EPI_SPLIT_RES:
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                  const float4 t = F_V(j);
+                  o[j] = to_c2 ? t : make_float4(a.c_old * x[j].x + t.x, a.c_old * x[j].y + t.y, a.c_old * x[j].z + t.z, a.c_old * x[j].w + t.w);
+                }
+                break;
+              default:
+#pragma unroll
+                for (int j = 0; j < 4; ++j) o[j] = F_V(j);
+                break;
             }
-          } break;
-          case EPI_Y_X:
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const float4 t = F_V(j);
-              o[j] = pass == 0 ? t : make_float4(u * t.x, u * t.y, u * t.z, u * t.w);
-            }
-            break;
-          case EPI_RESIDUAL:
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const float4 t = F_V(j);
-              o[j] = pass == 0 ? t
-                               : make_float4(a.c_old * x[j].x + cu * t.x, a.c_old * x[j].y + cu * t.y, a.c_old * x[j].z + cu * t.z,
-                                             a.c_old * x[j].w + cu * t.w);
-            }
-            break;
-          case EPI_DSILU:
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const float4 t = F_V(j);
-              o[j] = make_float4(t.x * dsilu_f(x[j].x), t.y * dsilu_f(x[j].y), t.z * dsilu_f(x[j].z), t.w * dsilu_f(x[j].w));
-            }
-            break;
-          case EPI_ACCUM:
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const float4 t = F_V(j);
-              o[j] = make_float4(x[j].x + t.x, x[j].y + t.y, x[j].z + t.z, x[j].w + t.w);
-            }
-            break;
-          case EPI_SPLIT_RES:
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const float4 t = F_V(j);
-              o[j] = to_c2 ? t : make_float4(a.c_old * x[j].x + t.x, a.c_old * x[j].y + t.y, a.c_old * x[j].z + t.z, a.c_old * x[j].w + t.w);
-            }
-            break;
-          default:
-#pragma unroll
-            for (int j = 0; j < 4; ++j) o[j] = F_V(j);
-            break;
-        }
 #undef F_V
 #pragma unroll
-        for (int j = 0; j < 4; ++j) *reinterpret_cast<float4*>(orow + ((j ^ sw) << 4)) = o[j];
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // tile stores -> visible to the TMA unit
-        asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
-        if (leader) {
-          const bool second = to_c2 || pass == 1;
-          const CUtensorMap* tm = second ? &tmC2 : &tmC;
-          const int cc = to_c2 ? nb - a.split : nb;
-          if (fa.c_d3 && !second) tma_store_3d(tm, cc, 0, mt * epb_c, obuf);
-          else tma_store_2d(tm, cc, (int)row0, obuf);
-          asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            for (int j = 0; j < 4; ++j) *reinterpret_cast<float4*>(orow + (((sub * 4 + j) ^ sw) << 4)) = o[j];
+          }
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // tile stores -> visible to the TMA unit
+          asm volatile("bar.sync %0, 128;" ::"r"(bar_id) : "memory");
+          if (leader) {
+            const bool second = to_c2 || pass == 1;
+            const CUtensorMap* tm = second ? &tmC2 : &tmC;
+            const int cc = to_c2 ? nb - a.split : nb;
+            if (fa.c_d3 && !second) tma_store_3d(tm, cc, 0, mt * epb_c, obuf);
+            else tma_store_2d(tm, cc, (int)row0, obuf);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+          }
         }
       }
       asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -522,14 +457,12 @@ EncodeTiledFn encode_fn() {
   return fn;
 }
 
-// fp32 matrix [rows][K] with leading dimension ld, boxes of box_cols columns x box_rows rows (32 columns: SWIZZLE_128B operand
-// stages; 16 columns: SWIZZLE_64B epilogue tiles), zero fill / clipping outside.
+// fp32 matrix [rows][K] with leading dimension ld, boxes of 32 columns x 128 rows, SWIZZLE_128B, zero fill / clipping outside.
 // d3 > 0: rows are (edge, m) pairs of one irrep of an [e][comp][c] tensor (A points at its first row): 3-D map (c, m, e) with
 // boxes of 32 x d3 x (128 / d3); od = comps per edge.  box_rows < 128 for the plain side of a mapped GEMM: a store must not
 // touch the rows of the next tile.
-bool make_map(Model* m, const float* A, int K, int ld, int64_t rows, int d3, int od, int box_rows, int box_cols, CUtensorMap* out) {
-  const std::array<int64_t, 6> key = {(int64_t)(uintptr_t)A, K, ld, rows, d3 + 16 * box_rows + 4096 * box_cols, od};
-  const CUtensorMapSwizzle swz = box_cols == 32 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B;
+bool make_map(Model* m, const float* A, int K, int ld, int64_t rows, int d3, int od, int box_rows, CUtensorMap* out) {
+  const std::array<int64_t, 6> key = {(int64_t)(uintptr_t)A, K, ld, rows, d3 + 16 * box_rows, od};
   auto it = m->tmaps.find(key);
   if (it != m->tmaps.end()) { std::memcpy(out, &it->second, sizeof(CUtensorMap)); return true; }
   EncodeTiledFn enc = encode_fn();
@@ -539,17 +472,17 @@ bool make_map(Model* m, const float* A, int K, int ld, int64_t rows, int d3, int
   if (d3 > 0) {
     cuuint64_t gdim[3] = {(cuuint64_t)K, (cuuint64_t)d3, (cuuint64_t)(rows / d3)};
     cuuint64_t gstr[2] = {(cuuint64_t)ld * 4, (cuuint64_t)od * ld * 4};
-    cuuint32_t box[3] = {(cuuint32_t)box_cols, (cuuint32_t)d3, (cuuint32_t)(F_M / d3)};
+    cuuint32_t box[3] = {(cuuint32_t)F_KS, (cuuint32_t)d3, (cuuint32_t)(F_M / d3)};
     cuuint32_t estr[3] = {1, 1, 1};
     r = enc(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(A), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-            swz, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   } else {
     cuuint64_t gdim[2] = {(cuuint64_t)K, (cuuint64_t)rows};
     cuuint64_t gstr[1] = {(cuuint64_t)ld * 4};
-    cuuint32_t box[2] = {(cuuint32_t)box_cols, (cuuint32_t)box_rows};
+    cuuint32_t box[2] = {(cuuint32_t)F_KS, (cuuint32_t)box_rows};
     cuuint32_t estr[2] = {1, 1};
     r = enc(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(A), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-            swz, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   }
   if (r != CUDA_SUCCESS) return false;
   TMapStore s;
@@ -587,7 +520,7 @@ bool launch_gemm_f16s(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t s
   if (a.ldc % 4 || !al(a.C)) return false;
   if (a.C2 && (a.ldc2 % 4 || !al(a.C2))) return false;
   if (a.aux && (a.ldaux % 4 || !al(a.aux))) return false;
-  if (a.epi == EPI_SPLIT_RES && a.split % 16) return false;
+  if (a.epi == EPI_SPLIT_RES && a.split % 32) return false;
   if (a.m_mul != 1 && (a.epi != EPI_STORE || a.pro != PRO_NONE)) return false;
   if ((a.amap_d3 || a.cmap_d3) && (a.K1 > 0 || a.epi != EPI_STORE)) return false;
   if (a.amap_d3 && a.cmap_d3 && a.amap_d3 != a.cmap_d3) return false;
@@ -611,54 +544,26 @@ bool launch_gemm_f16s(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t s
   fa.a_d3 = a.amap_d3; fa.c_d3 = a.cmap_d3;
   const int64_t rows_cap = m->f16_rows_cap * a.m_mul;                              // rows the operand buffers hold (workspace capacity)
   CUtensorMap t0, t1, tc, tc2;
-  if (a.amap_d3) { if (!make_map(m, a.A0 + (int64_t)a.amap_off * a.lda0, a.K0, a.lda0, rows_cap, a.amap_d3, a.amap_od, F_M, F_KS, &t0)) return false; }
-  else if (!make_map(m, a.A0, a.K0, a.lda0, rows_cap, 0, 0, F_M, F_KS, &t0)) return false;
-  if (a.K1 > 0) { if (!make_map(m, a.A1, a.K1, a.lda1, rows_cap, 0, 0, F_M, F_KS, &t1)) return false; }
+  if (a.amap_d3) { if (!make_map(m, a.A0 + (int64_t)a.amap_off * a.lda0, a.K0, a.lda0, rows_cap, a.amap_d3, a.amap_od, F_M, &t0)) return false; }
+  else if (!make_map(m, a.A0, a.K0, a.lda0, rows_cap, 0, 0, F_M, &t0)) return false;
+  if (a.K1 > 0) { if (!make_map(m, a.A1, a.K1, a.lda1, rows_cap, 0, 0, F_M, &t1)) return false; }
   else t1 = t0;
   const int cw = a.epi == EPI_SPLIT_RES ? a.split : a.N;
-  if (a.cmap_d3) { if (!make_map(m, a.C + (int64_t)a.cmap_off * a.ldc, cw, a.ldc, rows_cap, a.cmap_d3, a.cmap_od, F_M, 16, &tc)) return false; }
-  else if (!make_map(m, a.C, cw, a.ldc, rows_cap, 0, 0, fa.rpt, 16, &tc)) return false;
-  if (a.C2) { if (!make_map(m, a.C2, a.epi == EPI_SPLIT_RES ? a.N - a.split : a.N, a.ldc2, rows_cap, 0, 0, fa.rpt, 16, &tc2)) return false; }
+  if (a.cmap_d3) { if (!make_map(m, a.C + (int64_t)a.cmap_off * a.ldc, cw, a.ldc, rows_cap, a.cmap_d3, a.cmap_od, F_M, &tc)) return false; }
+  else if (!make_map(m, a.C, cw, a.ldc, rows_cap, 0, 0, fa.rpt, &tc)) return false;
+  if (a.C2) { if (!make_map(m, a.C2, a.epi == EPI_SPLIT_RES ? a.N - a.split : a.N, a.ldc2, rows_cap, 0, 0, fa.rpt, &tc2)) return false; }
   else tc2 = tc;
-  // auxiliary rows of the epilogue: the residual input / saved pre-activation (aux), or C itself for the accumulation
-  CUtensorMap tx = tc;
-  if (a.epi == EPI_ACCUM) { if (a.cmap_d3) return false; }
-  else if (a.epi == EPI_RESIDUAL || a.epi == EPI_DSILU || a.epi == EPI_SPLIT_RES) {
-    if (!a.aux || !make_map(m, a.aux, a.epi == EPI_SPLIT_RES ? a.split : a.N, a.ldaux, rows_cap, 0, 0, fa.rpt, 16, &tx)) return false;
-  }
   static int attr_dev = -1;
   if (attr_dev != m->device) {
     if (cudaFuncSetAttribute(k_gemm_f16s, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F_SMEM) != cudaSuccess) { cudaGetLastError(); return false; }
     attr_dev = m->device;
   }
-  fa.trace = nullptr;
-#ifdef F16S_TRACE
-  static unsigned long long* tr = nullptr;
-  if (!tr) cudaMalloc(&tr, 16 * 16 * 8);
-  cudaMemsetAsync(tr, 0, 16 * 16 * 8, st);
-  fa.trace = tr;
-#endif
   const int64_t tiles = ((m_cap * a.m_mul + fa.rpt - 1) / fa.rpt) * fa.n_nt;
   const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(tiles, m->num_sms));
   prof_begin(m, st, KC_GEMM16, 2.0 * a.N * K * a.m_mul);
-  k_gemm_f16s<<<grid, F_T, F_SMEM, st>>>(fa, t0, t1, tc, tc2, tx);
+  k_gemm_f16s<<<grid, F_T, F_SMEM, st>>>(fa, t0, t1, tc, tc2);
   prof_end(m, st);
   m->launches += 1;
-#ifdef F16S_TRACE
-  {   // developer build: print the timeline of CTA 0 (cycles)
-    unsigned long long hb[256];
-    cudaStreamSynchronize(st);
-    cudaMemcpy(hb, fa.trace, sizeof(hb), cudaMemcpyDeviceToHost);
-    std::printf("k_gemm_f16s K=%d N=%d pro=%d epi=%d\n", K, a.N, a.pro, a.epi);
-    for (int t = 2; t < 6; ++t) {
-      unsigned long long* q = hb + t * 16;
-      std::printf("  tile %d: mma wait_acc %6lld loop %6lld (wait cvt %6lld, wait b %6lld) | epi wait %6lld run %6lld (bar1 %lld fill %lld bar2 %lld) | cvt0 wait raw %6lld wait mma_done %6lld | period %lld\n",
-                  t, (long long)(q[1] - q[0]), (long long)(q[2] - q[1]), (long long)q[3], (long long)q[4], (long long)(q[6] - q[5]),
-                  (long long)(q[7] - q[6]), (long long)q[10], (long long)q[11], (long long)q[12], (long long)q[8], (long long)q[9],
-                  (long long)(q[0] - hb[(t - 1) * 16]));
-    }
-  }
-#endif
   return true;
 }
 
