@@ -113,6 +113,28 @@ int allegro_md_deform(void* h, const double* cell_new, void* stream);
 int allegro_set_state(void* h, const double* pos, const double* vel, void* stream);
 int allegro_virial(void* h, const double* pos, double* W_out, void* stream);
 
+/* spatial decomposition of the strictly local model (the property behind the paper's 0.964
+ * parallel efficiency on Aurora).  One process per GPU; coordinates are replicated on every rank, so the only collective of a
+ * step is one all-reduce of the force array and the 8-byte energy (paper_2502_06073_b200/distributed.py).
+ *  - allegro_energy_forces_owned: as allegro_energy_forces, but only atoms [0, n_owned) are centre atoms; atoms [n_owned, N) are
+ *    ghosts (neighbours only).  E = sum of E_i over the owned atoms, F_out [N,3] = -dE/dr of that partial sum for EVERY atom
+ *    (ghost rows hold the reaction forces that the owner rank adds up).
+ *  - allegro_decomp_select: local atom set of the brick `coord` of the rank grid `grid` (HOST int32 [3] each): owned atoms first
+ *    (wrapped position inside the brick in every decomposed dimension, ascending atom index), then every periodic image within
+ *    r_halo of the brick.  Writes local_pos DEVICE fp64 [cap,3] (coordinates inside the local box), local_species DEVICE int32
+ *    [cap] (may be NULL), local_src DEVICE int64 [cap] (global atom index), counts HOST int64 [2] = {n_owned, n_local},
+ *    local_cell HOST fp64 [3,3] (periodic as the global cell in undecomposed dimensions, padded and pair-free across its wrap in
+ *    decomposed ones).  Needs brick + 2 r_halo <= L in decomposed dimensions (an atom appears at most once per rank).
+ *  - allegro_decomp_scatter: F_global [N,3] = 0, then F_global[local_src[k]] = F_local[k] (conflict-free, deterministic).
+ *  - allegro_kick_drift: v += dt/2 a; if (drift) r += dt v on caller arrays (DEVICE fp64), a = 9.648533212e-3 F / m (A20). */
+int allegro_energy_forces_owned(void* h, const double* pos, const int32_t* species, int64_t N, const double* cell, int64_t n_owned,
+                                double* E_out, double* F_out, float* E_atom_out, void* stream);
+int allegro_decomp_select(void* h, const double* pos, const int32_t* species, int64_t N, const double* cell, const int32_t* grid,
+                          const int32_t* coord, double r_halo, int64_t cap, double* local_pos, int32_t* local_species, int64_t* local_src,
+                          int64_t* counts, double* local_cell, void* stream);
+int allegro_decomp_scatter(const double* F_local, const int64_t* local_src, int64_t n_local, double* F_global, int64_t N, void* stream);
+int allegro_kick_drift(double* pos, double* vel, const double* F, const double* mass, int64_t N, double dt_fs, int drift, void* stream);
+
 /* Copies the MD state out.  pos/vel/F DEVICE fp64 [N,3]; E_pot/E_kin DEVICE fp64 [1]; n_rebuilds HOST
  * int64 [1].  Any pointer may be NULL. */
 int allegro_get_state(void* h, double* pos, double* vel, double* F, double* E_pot, double* E_kin,

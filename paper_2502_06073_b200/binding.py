@@ -24,7 +24,8 @@ ERR_NAMES = {0: "OK", -1: "INVALID", -2: "UNSUPPORTED", -3: "CUDA", -4: "STALE_L
              -7: "SPECIES", -8: "NO_LIST", -9: "ALLOC"}
 EXPORTS = ["allegro_weight_layout", "allegro_create", "allegro_destroy", "allegro_build_neighbors",
            "allegro_energy_forces", "allegro_md_init", "allegro_md_step", "allegro_md_step_nvt", "allegro_md_deform",
-           "allegro_set_state", "allegro_virial", "allegro_debug_set_list_slack", "allegro_get_state",
+           "allegro_set_state", "allegro_virial", "allegro_debug_set_list_slack", "allegro_energy_forces_owned",
+           "allegro_decomp_select", "allegro_decomp_scatter", "allegro_kick_drift", "allegro_get_state",
            "allegro_get_neighbors", "allegro_get_stats", "allegro_profile", "allegro_get_profile",
            "allegro_debug_coupling", "allegro_debug_num_paths", "allegro_debug_set_precision", "allegro_debug_gemm",
            "allegro_last_error"]
@@ -60,6 +61,10 @@ _lib.allegro_md_deform.argtypes = [_vp, _vp, _vp]
 _lib.allegro_set_state.argtypes = [_vp, _vp, _vp, _vp]
 _lib.allegro_virial.argtypes = [_vp, _vp, _vp, _vp]
 _lib.allegro_debug_set_list_slack.argtypes = [_vp, _dbl, _i64]
+_lib.allegro_energy_forces_owned.argtypes = [_vp, _vp, _vp, _i64, _vp, _i64, _vp, _vp, _vp, _vp]
+_lib.allegro_decomp_select.argtypes = [_vp, _vp, _vp, _i64, _vp, _vp, _vp, _dbl, _i64, _vp, _vp, _vp, _vp, _vp, _vp]
+_lib.allegro_decomp_scatter.argtypes = [_vp, _vp, _i64, _vp, _i64, _vp]
+_lib.allegro_kick_drift.argtypes = [_vp, _vp, _vp, _vp, _i64, _dbl, C.c_int, _vp]
 _lib.allegro_get_state.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]
 _lib.allegro_get_neighbors.argtypes = [_vp, _vp, _vp, _vp, _vp]
 _lib.allegro_get_stats.argtypes = [_vp, _vp]
@@ -172,6 +177,21 @@ class Allegro:
         self._check(_lib.allegro_energy_forces(self._h, _ptr(pos), _ptr(species), pos.shape[0], c.ctypes.data,
                                                _ptr(E_out), _ptr(F_out), _ptr(E_atom_out), _stream()))
 
+    def energy_forces_owned(self, pos, species, cell, n_owned, E_out, F_out, E_atom_out=None):
+        c = self._cell_host(cell)
+        self._check(_lib.allegro_energy_forces_owned(self._h, _ptr(pos), _ptr(species), pos.shape[0], c.ctypes.data, int(n_owned),
+                                                     _ptr(E_out), _ptr(F_out), _ptr(E_atom_out), _stream()))
+
+    def decomp_select(self, pos, species, cell, grid, coord, r_halo, local_pos, local_species, local_src):
+        """-> (n_owned, n_local, local_cell [3,3]); the local arrays are caller tensors with capacity local_pos.shape[0]."""
+        c = self._cell_host(cell)
+        g = np.ascontiguousarray(grid, dtype=np.int32); k = np.ascontiguousarray(coord, dtype=np.int32)
+        counts = np.zeros(2, np.int64); lc = np.zeros((3, 3))
+        self._check(_lib.allegro_decomp_select(self._h, _ptr(pos), _ptr(species), pos.shape[0], c.ctypes.data, g.ctypes.data, k.ctypes.data,
+                                               float(r_halo), int(local_pos.shape[0]), _ptr(local_pos), _ptr(local_species), _ptr(local_src),
+                                               counts.ctypes.data, lc.ctypes.data, _stream()))
+        return int(counts[0]), int(counts[1]), lc
+
     def md_init(self, pos, vel, mass, species, cell, cutoff, skin):
         c = self._cell_host(cell)
         self._n_atoms = pos.shape[0]
@@ -262,6 +282,18 @@ class Allegro:
         self.energy_forces(pos, sp, cell, E, F, Ea)
         out = (float(E.item()), F.cpu().numpy())
         return out + ((Ea.cpu().numpy(),) if want_atom else ())
+
+
+def decomp_scatter(F_local, local_src, n_local, F_global):
+    rc = _lib.allegro_decomp_scatter(_ptr(F_local), _ptr(local_src), int(n_local), _ptr(F_global), F_global.shape[0], _stream())
+    if rc != 0:
+        raise AllegroError(rc, "allegro_decomp_scatter")
+
+
+def kick_drift(pos, vel, F, mass, dt_fs, drift):
+    rc = _lib.allegro_kick_drift(_ptr(pos), _ptr(vel), _ptr(F), _ptr(mass), pos.shape[0], float(dt_fs), 1 if drift else 0, _stream())
+    if rc != 0:
+        raise AllegroError(rc, "allegro_kick_drift")
 
 
 def build_weights(hp: dict, seed: int) -> np.ndarray:

@@ -235,7 +235,7 @@ int allegro_destroy(void* h) {
   NeighborList& nl = m->nl;
   for (DevBuf* b : {&nl.r_build, &nl.img, &nl.cell_of, &nl.cell_cnt, &nl.cell_start, &nl.cell_fill, &nl.sorted, &nl.row_cnt, &nl.rowptr,
                     &nl.keys_tmp, &nl.keys, &nl.revpos, &nl.scan_tmp, &m->ws.arena, &m->ws.scan_tmp, &m->g_list, &m->e_atom, &m->e_partial, &m->act_total,
-                    &m->flags, &m->md_pos, &m->md_vel, &m->md_mass, &m->md_species, &m->md_F, &m->md_E, &m->vir_partial, &m->nvt_par, &nl.rowptr_new})
+                    &m->flags, &m->md_pos, &m->md_vel, &m->md_mass, &m->md_species, &m->md_F, &m->md_E, &m->vir_partial, &m->nvt_par, &nl.rowptr_new, &m->decomp_tmp})
     free_buf(*b);
   delete m;
   return ALLEGRO_OK;
@@ -278,6 +278,48 @@ int allegro_energy_forces(void* h, const double* pos, const int32_t* species, in
   if (rc == ALLEGRO_ERR_ALLOC) { m->ws.slack *= 1.5; m->ws.for_N = -1; }   // a chunk overflowed its workspace share: a retry gets more
   m->stats[0] = act; m->stats[2] = m->launches; m->stats[3] = 0; m->stats[4] = 1;
   return rc;
+}
+
+int allegro_energy_forces_owned(void* h, const double* pos, const int32_t* species, int64_t N, const double* cell, int64_t n_owned,
+                                double* E_out, double* F_out, float* E_atom_out, void* stream) {
+  if (!h) return ALLEGRO_ERR_INVALID;
+  Model* m = static_cast<Model*>(h);
+  if (!pos || !species || !cell || !E_out || !F_out || n_owned < 0 || n_owned > N) { m->err = "allegro_energy_forces_owned: bad argument"; return ALLEGRO_ERR_INVALID; }
+  if (!m->nl.valid) { m->err = "allegro_energy_forces_owned called before allegro_build_neighbors"; return ALLEGRO_ERR_NO_LIST; }
+  if (N != m->nl.N) { m->err = "N differs from the neighbour list"; return ALLEGRO_ERR_INVALID; }
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  m->launches = 0;
+  int rc = network_energy_forces(m, pos, species, N, E_out, F_out, E_atom_out, st, n_owned);
+  if (rc) return rc;
+  int64_t act = 0;
+  if (N > 0 && m->act_total.p) cudaMemcpyAsync(&act, m->act_total.p, sizeof(int64_t), cudaMemcpyDeviceToHost, st);
+  rc = check_flags(m, st, "allegro_energy_forces_owned");
+  if (rc == ALLEGRO_ERR_ALLOC) { m->ws.slack *= 1.5; m->ws.for_N = -1; }
+  m->stats[0] = act; m->stats[2] = m->launches; m->stats[3] = 0; m->stats[4] = 1;
+  return rc;
+}
+
+int allegro_decomp_select(void* h, const double* pos, const int32_t* species, int64_t N, const double* cell, const int32_t* grid,
+                          const int32_t* coord, double r_halo, int64_t cap, double* local_pos, int32_t* local_species, int64_t* local_src,
+                          int64_t* counts, double* local_cell, void* stream) {
+  if (!h) return ALLEGRO_ERR_INVALID;
+  Model* m = static_cast<Model*>(h);
+  if ((!pos && N > 0) || !cell || !grid || !coord || !local_pos || !local_src || !counts || !local_cell || N < 0 || cap < 0 || !(r_halo > 0.0)) {
+    m->err = "allegro_decomp_select: bad argument"; return ALLEGRO_ERR_INVALID;
+  }
+  return decomp_select(m, pos, species, N, cell, grid, coord, r_halo, cap, local_pos, local_species, local_src, counts, local_cell,
+                       static_cast<cudaStream_t>(stream));
+}
+
+int allegro_decomp_scatter(const double* F_local, const int64_t* local_src, int64_t n_local, double* F_global, int64_t N, void* stream) {
+  if ((!F_local || !local_src) && n_local > 0) return ALLEGRO_ERR_INVALID;
+  if (!F_global && N > 0) return ALLEGRO_ERR_INVALID;
+  return decomp_scatter(F_local, local_src, n_local, F_global, N, static_cast<cudaStream_t>(stream));
+}
+
+int allegro_kick_drift(double* pos, double* vel, const double* F, const double* mass, int64_t N, double dt_fs, int drift, void* stream) {
+  if ((!pos || !vel || !F || !mass) && N > 0) return ALLEGRO_ERR_INVALID;
+  return ext_kick_drift(pos, vel, F, mass, N, dt_fs, drift, static_cast<cudaStream_t>(stream));
 }
 
 int allegro_md_init(void* h, const double* pos, const double* vel, const double* mass, const int32_t* species, int64_t N,

@@ -103,7 +103,7 @@ struct Model {
   NeighborList nl;
   Workspace ws;
   // global per-list-edge gradient and per-atom outputs
-  DevBuf g_list, e_atom, e_partial, act_total, flags, md_pos, md_vel, md_mass, md_species, md_F, md_E, vir_partial, nvt_par;
+  DevBuf g_list, e_atom, e_partial, act_total, flags, md_pos, md_vel, md_mass, md_species, md_F, md_E, vir_partial, nvt_par, decomp_tmp;
   bool md_ready = false;
   // CUDA-graph replay of one MD step (md.cu)
   bool use_graph = true, md_warm = false;
@@ -142,7 +142,14 @@ int nl_export(Model* m, int64_t* rowptr, int32_t* col, int8_t* shift, cudaStream
 // ---- network.cu
 int ws_prepare(Model* m, int64_t cap_edges, int64_t cap_atoms);
 int network_energy_forces(Model* m, const double* pos, const int32_t* species, int64_t N,
-                          double* E_out, double* F_out, float* E_atom_out, cudaStream_t st);
+                          double* E_out, double* F_out, float* E_atom_out, cudaStream_t st, int64_t n_owned = -1);
+
+// ---- decomp.cu
+int decomp_select(Model* m, const double* pos, const int32_t* species, int64_t N, const double* cell, const int32_t* grid, const int32_t* coord,
+                  double r_halo, int64_t cap, double* lpos, int32_t* lspecies, int64_t* lsrc, int64_t* counts_host, double* local_cell_host,
+                  cudaStream_t st);
+int decomp_scatter(const double* F_local, const int64_t* lsrc, int64_t n_local, double* F_global, int64_t N, cudaStream_t st);
+int ext_kick_drift(double* pos, double* vel, const double* F, const double* mass, int64_t N, double dt, int drift, cudaStream_t st);
 
 // ---- md.cu
 int md_init(Model* m, const double* pos, const double* vel, const double* mass, const int32_t* species, int64_t N,

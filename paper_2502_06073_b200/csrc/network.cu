@@ -464,8 +464,9 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
 }
 
 int network_energy_forces(Model* m, const double* pos, const int32_t* species, int64_t N, double* E_out, double* F_out,
-                          float* E_atom_out, cudaStream_t st) {
+                          float* E_atom_out, cudaStream_t st, int64_t n_owned) {
   NeighborList& nl = m->nl;
+  if (n_owned < 0 || n_owned > N) n_owned = N;                 // centre atoms [0, n_owned); the rest are ghosts (neighbours only)
   int* flags = m->flags.as<int>();
   if (int rc = ensure(m, &m->e_atom, sizeof(float) * (N + 1))) return rc;
   if (int rc = ensure(m, &m->e_partial, sizeof(double) * 1024)) return rc;
@@ -495,8 +496,13 @@ int network_energy_forces(Model* m, const double* pos, const int32_t* species, i
     ws.for_N = N; ws.for_cap = Ecap; ws.atoms_per = std::max<int64_t>(atoms_per, 1);
   }
   const int64_t atoms_per = ws.atoms_per;
-  for (int64_t a0 = 0; a0 < N; a0 += atoms_per) {
-    const int64_t a1 = std::min(N, a0 + atoms_per);
+  if (n_owned < N) {
+    // rows of the ghost atoms are not evaluated: their per-edge gradients and energies must read as zero
+    cudaMemsetAsync(m->g_list.p, 0, sizeof(float) * 3 * (size_t)std::max<int64_t>(nl.cap, 1), st);
+    cudaMemsetAsync(m->e_atom.p, 0, sizeof(float) * (N + 1), st);
+  }
+  for (int64_t a0 = 0; a0 < n_owned; a0 += atoms_per) {
+    const int64_t a1 = std::min(n_owned, a0 + atoms_per);
     if (int rc = run_chunk(m, pos, species, a0, a1, m->ws.cap_edges, st)) return rc;
   }
   ListView lv{nl.rowptr.as<int64_t>(), nl.keys.as<uint64_t>(), nl.revpos.as<int>(), {nl.L[0], nl.L[1], nl.L[2]}};
@@ -504,7 +510,7 @@ int network_energy_forces(Model* m, const double* pos, const int32_t* species, i
     prof_begin(m, st, KC_GATHER, 0);
     k_force_gather<<<(unsigned)((N * 32 + T - 1) / T), T, 0, st>>>(lv, N, m->g_list.as<float>(), F_out, flags);
     const int nb = (int)std::min<int64_t>(1024, (N + 255) / 256);
-    k_energy_partial<<<nb, 256, 0, st>>>(m->e_atom.as<float>(), N, m->e_partial.as<double>());
+    k_energy_partial<<<nb, 256, 0, st>>>(m->e_atom.as<float>(), n_owned, m->e_partial.as<double>());
     k_energy_final<<<1, 256, 0, st>>>(m->e_partial.as<double>(), nb, E_out, flags);
     prof_end(m, st);
     m->launches += 3;
