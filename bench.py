@@ -47,6 +47,9 @@ def parse():
     ap.add_argument("--log2n", type=int, default=15, help="size for --config 4")
     ap.add_argument("--md-steps", type=int, default=0, help="MD steps per bench step (default: the config's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--decomp", action="store_true",
+                    help="N > 1: ONE system decomposed over the ranks (paper_2502_06073_b200/distributed.py, strong scaling) instead of "
+                         "the default independent replicas")
     ap.add_argument("--sample-atoms", type=int, default=0, help="reference arm: centre atoms per step")
     return ap.parse_args()
 
@@ -215,12 +218,13 @@ def roofline_for(prof, stats, clocks, peaks, n_sm, n_atoms, ms_md_step):
     except Exception:
         pass
     if dom in flops:
+        n_l = prof[dom].get("launches_per_md_step", prof[dom]["launches"])
         ach = flops[dom] / (prof[dom]["ms"] * 1e-3) / 1e12
         peak = {"gemm": peak_tf32x3, "gemm_f16s": peak_f16s}.get(dom, fp32_peak)
         roof.update({"bound": "tensor" if dom.startswith("gemm") else "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
-                     "frac": ach / peak, "traffic": traffic, "traffic_source": traffic_src, "launches": prof[dom]["launches"],
-                     "avg_launch_ms": prof[dom]["ms"] / max(1, prof[dom]["launches"]),
-                     "algorithmic_flop_per_launch": flops[dom] / max(1, prof[dom]["launches"]),
+                     "frac": ach / peak, "traffic": traffic, "traffic_source": traffic_src, "launches_per_md_step": n_l,
+                     "avg_launch_ms": prof[dom]["ms"] / max(1, n_l),
+                     "algorithmic_flop_per_launch": flops[dom] / max(1, n_l),
                      "peak_source": {"gemm": t16_src + " x 1.1/2.25 (nominal TF32:BF16) / 3 passes (3xTF32 split, gemm_tc.cu)",
                                      "gemm_f16s": t16_src + " / 3 passes (split-fp16 product hi*hi + hi*lo + lo*hi, gemm_f16s.cu)"}.get(
                                          dom, "148 SM x 128 FP32 lanes x 2 x clocks.max.sm (DESIGN.md)")})
@@ -332,6 +336,8 @@ def run_ours(args):
     model.md_step(w.dt_fs, n_md)
     prof = model.get_profile()
     model.profile(False)
+    for v in prof.values():                       # per MD step: the profiled call ran n_md of them
+        v["ms"] /= n_md; v["work"] /= n_md; v["launches_per_md_step"] = v["launches"] / n_md
 
     ms, ms_e2e = max_over_ranks([ms, ms_e2e], world, "cuda")
     if rank != 0:
@@ -383,6 +389,52 @@ def run_ours(args):
                                 "sample": f"{reps} oracle energy+force evaluations (fp64 numpy, as it stands) over {ns} seeded centre "
                                           f"atoms of {w.name} with their full neighbourhoods, {tsum:.1f} s of wall time; cores = CPU time / wall time"}
     print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_decomp(args):
+    """--decomp: one system, spatially decomposed over the ranks.  value = atoms * n_md * steps / time (strong
+    scaling: total work fixed).  The one collective of a step is the all-reduce of the force array over NCCL."""
+    import torch
+    import torch.distributed as dist
+    from paper_2502_06073_b200 import binding as B
+    from paper_2502_06073_b200.distributed import DistributedAllegro
+    world = int(os.environ.get("WORLD_SIZE", "1")); rank = int(os.environ.get("RANK", "0")); local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    WL, w, n_md = load_workload(args)
+    N = w.n_atoms
+    d = DistributedAllegro(B.build_weights(w.hp, w.weight_seed), w.hp, w.cell, rank=rank, world=world)
+    vel0 = WL.maxwell_boltzmann(w.mass, w.temperature, w.vel_seed)
+    dev = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a, dtype=dt)).cuda()
+    pos, vel, mass, sp = dev(w.pos, np.float64), dev(vel0, np.float64), dev(w.mass, np.float64), dev(w.species, np.int32)
+    F = torch.zeros((N, 3), dtype=torch.float64, device="cuda")
+    d.energy_forces(pos, sp, F)
+    for _ in range(args.warmup):
+        d.md_step(pos, vel, mass, sp, F, w.dt_fs, n_md)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(args.steps):
+        E = d.md_step(pos, vel, mass, sp, F, w.dt_fs, n_md)
+    ev1.record()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ms, = max_over_ranks([ev0.elapsed_time(ev1)], world, "cuda")
+    if rank == 0:
+        value = N * n_md * args.steps / (ms * 1e-3)
+        print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                          "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+                          "dtype": "f32", "data": "synthetic",
+                          "config": config_dict(w, n_md, {"parallelism": "spatial decomposition %dx%dx%d, replicated coordinates, one force "
+                                                                         "all-reduce per step" % d.grid,
+                                                          "owned_atoms_rank0": d.n_owned, "local_atoms_rank0": d.n_local}),
+                          "E_pot": float(E.item())}))
     if world > 1:
         dist.destroy_process_group()
 
@@ -446,6 +498,8 @@ def main():
         run_reference(args)
     elif args.sweep:
         run_sweep(args)
+    elif args.decomp:
+        run_decomp(args)
     else:
         run_ours(args)
 

@@ -258,7 +258,7 @@ def config3() -> Workload:
                     notes="FM-sized network, 8 of 89 species, jittered FCT lattice (BASELINE.json configs[3])")
 
 
-_CFG4_TILINGS = {15: (2, 2, 2), 17: (4, 4, 2), 19: (8, 4, 4), 21: (8, 8, 8), 23: (16, 16, 8),
+_CFG4_TILINGS = {15: (2, 2, 2), 17: (4, 4, 2), 19: (8, 4, 4), 21: (8, 8, 8), 23: (16, 16, 8), 26: (32, 32, 16),
                  25: (32, 16, 16), 27: (32, 32, 32)}
 
 
