@@ -22,8 +22,13 @@ if os.environ.get("ALLEGRO_F16S_DBGWAIT"):   # developer build: barrier waits ti
     NVCC_FLAGS.append("-DF16S_DBGWAIT")
 
 
+STAMP = os.path.join(HERE, "build", "flags.txt")
+
+
 def _stale() -> bool:
     if not os.path.exists(LIB):
+        return True
+    if not os.path.exists(STAMP) or open(STAMP).read() != " ".join(NVCC_FLAGS):   # a developer build is replaced by a normal one
         return True
     t = os.path.getmtime(LIB)
     deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(HERE, "..", "include", "allegro.h"), __file__]
@@ -60,6 +65,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     r = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
     if r.returncode != 0:
         raise RuntimeError("link failed:\n" + r.stdout)
+    with open(STAMP, "w") as f:
+        f.write(" ".join(NVCC_FLAGS))
     return LIB
 
 

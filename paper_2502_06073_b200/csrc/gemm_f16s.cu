@@ -86,11 +86,11 @@ struct FArgs {
 #else
 #define TR_DECL
 #define TR_WAIT(i, stmt) { stmt; }
-#define TR_FLUSH(base)
+#define TR_FLUSH(base) {}
 #endif
 
 // bounded wait: a protocol error ends in a trap (sticky CUDA error) instead of a hung GPU
-__device__ __forceinline__ void mbar_wait_b(uint64_t* bar, uint32_t parity) {
+__device__ __forceinline__ void mbar_wait_l(uint64_t* bar, uint32_t parity, int line) {
   uint32_t done = 0;
   for (uint32_t it = 0; !done; ++it) {
     asm volatile(
@@ -100,9 +100,15 @@ __device__ __forceinline__ void mbar_wait_b(uint64_t* bar, uint32_t parity) {
         : "=r"(done)
         : "r"(smem_u32(bar)), "r"(parity), "r"(1000u)
         : "memory");
-    if (it > (1u << 22)) __trap();
+    if (it > (1u << 22)) {
+#ifdef F16S_DBGWAIT
+      printf("[f16s] wait timed out: line %d block %d warp %d parity %u\n", line, (int)blockIdx.x, (int)(threadIdx.x >> 5), parity);
+#endif
+      __trap();
+    }
   }
 }
+#define mbar_wait_b(bar, parity) mbar_wait_l(bar, parity, __LINE__)
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
