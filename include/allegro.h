@@ -113,6 +113,20 @@ int allegro_md_deform(void* h, const double* cell_new, void* stream);
 int allegro_set_state(void* h, const double* pos, const double* vel, void* stream);
 int allegro_virial(void* h, const double* pos, double* W_out, void* stream);
 
+/* allegro_virial for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): same arguments, same quantity (the summation order of the fp64 reduction differs, so the last bits may), but
+ *  - the call contains no cudaMalloc / cudaFree / allocating library routine and no stream synchronisation: two kernel launches
+ *    on `stream`, asynchronous; W_out is valid once the stream has reached that point, and an execution error surfaces at the
+ *    caller's next synchronisation;
+ *  - the block partials live in a fixed 288 KB file-scope __device__ array (held by every GPU that loads the library until the
+ *    process exits), which bounds the size: N > ALLEGRO_VIRIAL_NOALLOC_MAX_ATOMS returns ALLEGRO_ERR_UNSUPPORTED with a message
+ *    naming the limit (use allegro_virial then);
+ *  - every call on a device shares that array: calls that OVERLAP on the GPU (different streams or handles) race; calls on one
+ *    stream are safe.  The array keeps the last call's contents; every entry a call reads it has written first.
+ * The handle's device must be the current device on the first call per device (allegro_create does that call's set-up). */
+#define ALLEGRO_VIRIAL_NOALLOC_MAX_ATOMS 1048576
+int allegro_virial_noalloc(void* h, const double* pos, double* W_out, void* stream);
+
 /* spatial decomposition of the strictly local model (the property behind the paper's 0.964
  * parallel efficiency on Aurora).  One process per GPU; coordinates are replicated on every rank, so the only collective of a
  * step is one all-reduce of the force array and the 8-byte energy (paper_2502_06073_b200/distributed.py).

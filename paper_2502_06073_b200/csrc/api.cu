@@ -147,6 +147,7 @@ int allegro_create(const float* weights_host, size_t n_weights, const allegro_hp
   cudaGetDevice(&m->device);
   m->use_big = m->use_tc && m->use_tp3 && (hp->n_channels == 64 || hp->n_channels == 128 || hp->n_channels == 256);
   cudaDeviceGetAttribute(&m->num_sms, cudaDevAttrMultiProcessorCount, m->device);
+  virial_noalloc_setup(m);   // address lookup only; a failure is reported by allegro_virial_noalloc itself
   auto fail = [&](int rc, const std::string& msg) { g_create_err = msg; allegro_destroy(m); return rc; };
   if (cudaMalloc(&m->d_w, sizeof(float) * std::max<size_t>(n_weights, 1)) != cudaSuccess) return fail(ALLEGRO_ERR_ALLOC, "weights allocation failed");
   {

@@ -131,6 +131,9 @@ void prof_end(Model* m, cudaStream_t st);
 int ensure(Model* m, DevBuf* b, size_t bytes);            // grow-only cudaMalloc; 0 or ALLEGRO_ERR_ALLOC
 int cuda_fail(Model* m, cudaError_t e, const char* what);  // records message, returns ALLEGRO_ERR_CUDA
 
+// ---- virial_noalloc.cu: looks up the device address of the fixed scratch array (once per device, that device current)
+int virial_noalloc_setup(Model* m);
+
 // ---- scan.cu: exclusive scan of n int32 counts into n+1 int64 offsets (device), optionally conditional on *flag != 0
 int scan_counts(Model* m, const int* cnt, int64_t* out, int64_t n, DevBuf* tmp, const int* flag, cudaStream_t st);
 
