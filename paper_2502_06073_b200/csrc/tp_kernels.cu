@@ -1,5 +1,7 @@
 // tp_kernels.cu — instantiations of the generated tensor-product kernels (tp.cuh, tp3.cuh) and their launchers, in a
 // translation unit of their own: one instantiation per layer signature of tp_gen.cuh.
+#include <algorithm>
+
 #include "tp_big.cuh"
 
 namespace allegro {
@@ -72,13 +74,34 @@ size_t tpbig_floats_per_edge(const TpLayerDev& tp) {
   return f;
 }
 
+// backward: the ring kernel (T-bar staged by bulk copies) when at least two slots fit into shared memory, else k_tpo_bwd
+template <int SIG>
+bool launch_tpo_bwd_ring(cudaStream_t st, const TpLayerDev& tp, const TpIo& io, const TpBig& big) {
+  static int sms[64] = {0};
+  static bool attr[64] = {false};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return false;
+  if (!tp.has_lin || tp.n > 256 || 256 % tp.n) return false;
+  const size_t slot = TpoRing<SIG>::SLOT;
+  int n_slots = (int)std::min<size_t>(TPO_RING_MAX_SLOTS, (220 * 1024 - 128) / slot);
+  if (n_slots < 2) return false;
+  const size_t smem = (size_t)n_slots * slot + 128;
+  if (!attr[dev]) {
+    if (cudaFuncSetAttribute(k_tpo_bwd_ring<SIG>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024) != cudaSuccess) { cudaGetLastError(); return false; }
+    cudaDeviceGetAttribute(&sms[dev], cudaDevAttrMultiProcessorCount, dev);
+    attr[dev] = true;
+  }
+  k_tpo_bwd_ring<SIG><<<(unsigned)std::max(1, sms[dev]), TPO_RING_T, smem, st>>>(tp, io, big, n_slots);
+  return true;
+}
+
 void launch_tpo(int sig, bool backward, int64_t m_cap, cudaStream_t st, const TpLayerDev& tp, const TpIo& io, const TpBig& big) {
   const unsigned grid = (unsigned)((m_cap * tp.n + 255) / 256);
   switch (sig) {
-#define X(I)                                                                 \
-  case I:                                                                    \
-    if (!backward) k_tpo_fwd<I><<<grid, 256, 0, st>>>(tp, io, big);         \
-    else k_tpo_bwd<I><<<grid, 256, 0, st>>>(tp, io, big);                   \
+#define X(I)                                                                                         \
+  case I:                                                                                            \
+    if (!backward) k_tpo_fwd<I><<<grid, 256, 0, st>>>(tp, io, big);                                 \
+    else if (!launch_tpo_bwd_ring<I>(st, tp, io, big)) k_tpo_bwd<I><<<grid, 256, 0, st>>>(tp, io, big); \
     break;
     TPGEN_FOR_EACH_SIG(X)
 #undef X
