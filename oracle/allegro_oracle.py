@@ -312,11 +312,40 @@ def unpack_weights(hp, blob):
 # ================================================================================================
 # neighbours                                                                         (A16, A17)
 # ================================================================================================
-def _cell_lengths(cell):
-    cell = np.asarray(cell, dtype=np.float64)
-    if np.abs(cell - np.diag(np.diag(cell))).max() != 0.0:
-        raise ValueError("orthorhombic cells only")
-    return np.diag(cell).copy()
+def _cell_matrix(cell):
+    """H [3,3], rows = lattice vectors a_1, a_2, a_3 (reading A27): a periodic image is x + s_1 a_1 + s_2 a_2 + s_3 a_3."""
+    H = np.asarray(cell, dtype=np.float64).reshape(3, 3)
+    if not np.linalg.det(H) > 0.0:
+        raise ValueError("cell must be right-handed with positive volume")
+    return H
+
+
+def _is_diag(H):
+    return np.abs(H - np.diag(np.diag(H))).max() == 0.0
+
+
+def _image_shift(s, H):
+    """Cartesian shift of image s [..., 3]: (s_1 a_1 + s_2 a_2) + s_3 a_3, in this order (A27).  For a diagonal H the two
+    added terms are exact zeros, so the value is s_d L_d bit for bit, the expression of A16."""
+    s = np.asarray(s, dtype=np.float64)
+    return (s[..., 0:1] * H[0] + s[..., 1:2] * H[1]) + s[..., 2:3] * H[2]
+
+
+def cell_widths(cell):
+    """Perpendicular widths of the cell: the distance between the lattice planes f_d = 0 and f_d = 1 of the fractional
+    coordinate f = x H^-1, w_d = 1 / |column d of H^-1|.  For an orthorhombic cell these are the box lengths."""
+    H = _cell_matrix(cell)
+    if _is_diag(H):
+        return np.diag(H).copy()
+    Hinv = np.linalg.inv(H)
+    return 1.0 / np.sqrt((Hinv * Hinv).sum(axis=0))
+
+
+def _fractional(x, H):
+    """x H^-1 (x / L for a diagonal H, the expression the orthorhombic pins were made with)."""
+    if _is_diag(H):
+        return x / np.diag(H)
+    return x @ np.linalg.inv(H)
 
 
 def neighbors_bruteforce(pos, cell, radius, rows=None):
@@ -328,9 +357,9 @@ def neighbors_bruteforce(pos, cell, radius, rows=None):
     shift int32 [E,3]) with each row sorted by (j, sx, sy, sz).  ``rows``: only these centre atoms (CSR over
     them, in the given order) - the same loop body, used to sample rows of systems too large for N^2."""
     pos = np.asarray(pos, dtype=np.float64)
-    Ld = _cell_lengths(cell)
-    if radius > Ld.min():
-        raise ValueError("radius exceeds the smallest box length")
+    H = _cell_matrix(cell)
+    if radius > cell_widths(cell).min():
+        raise ValueError("radius exceeds the smallest box length (perpendicular width of the cell)")
     N = pos.shape[0]
     R2 = radius * radius
     centres = np.arange(N) if rows is None else np.asarray(rows)
@@ -338,9 +367,9 @@ def neighbors_bruteforce(pos, cell, radius, rows=None):
     trip = np.array([(a, b, c) for a in (-1, 0, 1) for b in (-1, 0, 1) for c in (-1, 0, 1)], dtype=np.int64)
     for q, i in enumerate(centres):
         d0 = pos - pos[i]                                   # x_j - x_i
-        n0 = -np.round(d0 / Ld).astype(np.int64)            # image bringing j closest to i
+        n0 = -np.round(_fractional(d0, H)).astype(np.int64)  # image bringing j closest to i (in fractional coordinates)
         s = n0[:, None, :] + trip[None, :, :]               # [N,27,3]
-        dx = d0[:, None, :] + s * Ld                        # (x_j - x_i) + s L
+        dx = d0[:, None, :] + _image_shift(s, H)            # (x_j - x_i) + s L   (A16; A27 for a general cell)
         d2 = dx[..., 0] * dx[..., 0] + dx[..., 1] * dx[..., 1] + dx[..., 2] * dx[..., 2]
         ok = d2 < R2
         ok[i] &= np.any(s[i] != 0, axis=1)                  # drop (i,i,0)
@@ -358,16 +387,22 @@ def neighbors_binned(pos, cell, radius):
     """Same set as neighbors_bruteforce, with candidates from a coarse grid (for the larger configs).
     The accept test is the identical fp64 expression; only the candidate enumeration differs."""
     pos = np.asarray(pos, dtype=np.float64)
-    Ld = _cell_lengths(cell)
+    H = _cell_matrix(cell)
+    Ld = cell_widths(cell)
     if radius > Ld.min():
-        raise ValueError("radius exceeds the smallest box length")
+        raise ValueError("radius exceeds the smallest box length (perpendicular width of the cell)")
     N = pos.shape[0]
     R2 = radius * radius
     nc = np.maximum(1, np.floor(Ld / (radius * (1 + 1e-9))).astype(np.int64))
-    h = Ld / nc
-    w = np.floor(pos / Ld).astype(np.int64)
-    xt = pos - w * Ld
-    ci = np.clip((xt / h).astype(np.int64), 0, nc - 1)
+    if _is_diag(H):
+        h = Ld / nc
+        w = np.floor(pos / Ld).astype(np.int64)
+        xt = pos - w * Ld
+        ci = np.clip((xt / h).astype(np.int64), 0, nc - 1)
+    else:                                                     # bins in fractional coordinates: every point within radius of x
+        f = _fractional(pos, H)                               # has |delta f_d| <= radius / width_d <= 1 / nc_d
+        w = np.floor(f).astype(np.int64)
+        ci = np.clip(((f - w) * nc).astype(np.int64), 0, nc - 1)
     cid = (ci[:, 0] * nc[1] + ci[:, 1]) * nc[2] + ci[:, 2]
     order = np.argsort(cid, kind="stable")
     start = np.searchsorted(cid[order], np.arange(nc.prod() + 1))
@@ -383,7 +418,7 @@ def neighbors_binned(pos, cell, radius):
         k = np.arange(cnt.sum()) - np.repeat(np.cumsum(cnt) - cnt, cnt)
         j = order[np.repeat(lo, cnt) + k]
         s = img[i_rep] + w[i_rep] - w[j]
-        dx = (pos[j] - pos[i_rep]) + s * Ld
+        dx = (pos[j] - pos[i_rep]) + _image_shift(s, H)
         d2 = dx[:, 0] * dx[:, 0] + dx[:, 1] * dx[:, 1] + dx[:, 2] * dx[:, 2]
         ok = (d2 < R2) & ~((i_rep == j) & np.all(s == 0, axis=1))
         ii_all.append(i_rep[ok]); jj_all.append(j[ok]); ss_all.append(s[ok])
@@ -450,8 +485,7 @@ class AllegroOracle:
         S, Nb, n, lmax, NL, p = hp["n_species"], hp["n_bessel"], hp["n_channels"], hp["lmax"], hp["n_layers"], hp["poly_p"]
         rc, navg = hp["r_cut"], hp["avg_num_neighbors"]
         inv_sqrt_n = 1.0 / math.sqrt(navg)
-        Ld = _cell_lengths(cell)
-        rvec = (pos[cj] - pos[ci]) + cs * Ld
+        rvec = (pos[cj] - pos[ci]) + _image_shift(cs, _cell_matrix(cell))
         r = np.sqrt(rvec[:, 0] * rvec[:, 0] + rvec[:, 1] * rvec[:, 1] + rvec[:, 2] * rvec[:, 2])
         Ne = r.shape[0]
         rhat = rvec / r[:, None]
@@ -600,7 +634,7 @@ class AllegroOracle:
         species = np.asarray(species)
         rowptr, col, shift = nbr
         N = pos.shape[0]
-        Ld = _cell_lengths(cell)
+        H = _cell_matrix(cell)
         rc2 = self.hp["r_cut"] ** 2
         centres = np.arange(N) if centres is None else np.asarray(centres)
         E_atom = np.zeros(N)
@@ -618,7 +652,7 @@ class AllegroOracle:
             ci = np.repeat(cc, [rowptr[a + 1] - rowptr[a] for a in cc])
             cj = col[idx].astype(np.int64)
             cs = shift[idx].astype(np.float64)
-            dx = (pos[cj] - pos[ci]) + cs * Ld
+            dx = (pos[cj] - pos[ci]) + _image_shift(cs, H)
             d2 = dx[:, 0] * dx[:, 0] + dx[:, 1] * dx[:, 1] + dx[:, 2] * dx[:, 2]
             act = d2 < rc2
             ci, cj, cs, loc, dxa = ci[act], cj[act], cs[act], loc[act], dx[act]
@@ -645,14 +679,19 @@ class AllegroOracle:
 def stress(virial, cell):
     """Cauchy stress of the potential part [eV/A^3]: sigma_ab = (1/V) dE/d eps_ab = -W_ab / V for the homogeneous
     strain r -> (1 + eps) r, cell -> (1 + eps) cell (PAPER.md:69 tensile test, :93/:112 stress in the training loss)."""
-    return -np.asarray(virial) / float(np.prod(_cell_lengths(cell)))
+    return -np.asarray(virial) / float(np.linalg.det(_cell_matrix(cell)))
 
 
 def md_deform(pos, cell, cell_new):
-    """A26: affine remap of the (unwrapped) positions from ``cell`` to ``cell_new`` (both orthorhombic):
-    x' = x L'_x / L_x.  The applied strain of PAPER.md:69 is a sequence of such increments between MD segments."""
-    L, Ln = _cell_lengths(cell), _cell_lengths(cell_new)
-    return np.asarray(pos, dtype=np.float64) * (Ln / L), np.diag(Ln)
+    """A26: affine remap of the (unwrapped) positions from ``cell`` to ``cell_new``: the fractional coordinates are kept,
+    x' = x H^-1 H'  (x' = x L'_x / L_x when both cells are orthorhombic).  The applied strain of PAPER.md:69 is a sequence of
+    such increments between MD segments."""
+    H, Hn = _cell_matrix(cell), _cell_matrix(cell_new)
+    pos = np.asarray(pos, dtype=np.float64)
+    if _is_diag(H) and _is_diag(Hn):
+        return pos * (np.diag(Hn) / np.diag(H)), np.diag(np.diag(Hn))
+    A = np.linalg.inv(H) @ Hn
+    return (pos[:, 0:1] * A[0] + pos[:, 1:2] * A[1]) + pos[:, 2:3] * A[2], Hn.copy()
 
 
 # ================================================================================================
