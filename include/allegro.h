@@ -20,8 +20,11 @@
  *    There is no host synchronisation inside the step loop of allegro_md_step except the one-word
  *    read-back that sizes a rebuilt neighbour list.
  *  - Units: Angstrom, fs, amu, eV.  Positions / velocities / masses / cell are fp64; the network runs
- *    in fp32.  Cells are orthorhombic (row vectors, off-diagonals must be 0) — triclinic cells return
- *    ALLEGRO_ERR_UNSUPPORTED.
+ *    in fp32.  A cell is a HOST fp64 [3,3] matrix whose ROWS are the lattice vectors a_1, a_2, a_3 (right-handed, det > 0;
+ *    else ALLEGRO_ERR_INVALID): orthorhombic (diagonal) or general / triclinic (reading A27 of DESIGN.md).  A
+ *    periodic image is x + s_1 a_1 + s_2 a_2 + s_3 a_3; cutoff + skin must not exceed the smallest perpendicular width of the
+ *    cell (the box lengths of an orthorhombic cell; ALLEGRO_ERR_CUTOFF).  Only the spatial decomposition (allegro_decomp_select)
+ *    still needs an orthorhombic cell.
  *  - There is no CPU fallback: without a CUDA device every compute call returns ALLEGRO_ERR_CUDA.
  */
 #ifndef ALLEGRO_B200_H
@@ -37,7 +40,7 @@ extern "C" {
 enum {
   ALLEGRO_OK = 0,
   ALLEGRO_ERR_INVALID = -1,      /* bad argument / hyper-parameters / weight count                   */
-  ALLEGRO_ERR_UNSUPPORTED = -2,  /* non-orthorhombic cell, lmax > 3, a row longer than the kernel cap  */
+  ALLEGRO_ERR_UNSUPPORTED = -2,  /* lmax > 3, a row longer than the kernel cap, decomposition of a triclinic cell */
   ALLEGRO_ERR_CUDA = -3,         /* CUDA runtime error (message has the cudaGetErrorString text)       */
   ALLEGRO_ERR_STALE_LIST = -4,   /* some atom moved more than skin/2 since allegro_build_neighbors     */
   ALLEGRO_ERR_NONFINITE = -5,    /* NaN/Inf detected in E or F                                         */
@@ -76,8 +79,9 @@ int allegro_destroy(void* h);
 
 /* Row a-1: device cell-list neighbour builder.  pos DEVICE fp64 [N,3] (unwrapped), species DEVICE int32
  * [N], cell HOST fp64 [3,3].  Builds the sorted CSR list of all ordered (i, j, s) with
- * |r_j + s.cell - r_i|^2 < (cutoff+skin)^2 evaluated in fp64 as dx = (x_j-x_i)+s_x*L_x, d2=dx*dx+dy*dy+dz*dz
- * (A16), (i,j,s) != (i,i,0), each row sorted by (j, sx, sy, sz).  cutoff must equal hp.r_cut. */
+ * |r_j + s.cell - r_i|^2 < (cutoff+skin)^2 evaluated in fp64 as dx = (x_j-x_i) + ((s_1*a_1x + s_2*a_2x) + s_3*a_3x)
+ * (= (x_j-x_i)+s_x*L_x bit for bit when the cell is diagonal), d2=dx*dx+dy*dy+dz*dz (A16, A27), (i,j,s) != (i,i,0), each row
+ * sorted by (j, s_1, s_2, s_3).  cutoff must equal hp.r_cut. */
 int allegro_build_neighbors(void* h, const double* pos, const int32_t* species, int64_t N,
                             const double* cell, double cutoff, double skin, void* stream);
 
@@ -101,7 +105,8 @@ int allegro_md_step(void* h, double dt_fs, int64_t n_steps, void* stream);
  *  - allegro_md_step_nvt: velocity-Verlet as allegro_md_step plus Berendsen weak coupling after the second half-kick of step
  *    k = 1..n_steps of this call: T_inst = 2 E_kin / ((3N-3) kB), T_target = T0 + (T1-T0) min(1, k/n_ramp) (n_ramp = 0: T1 at
  *    once), v <- v sqrt(1 + (dt/tau)(T_target/T_inst - 1)).  tau_fs >= dt_fs.  Deterministic; no host sync in the loop.
- *  - allegro_md_deform: affine remap of the unwrapped positions to cell_new (HOST fp64 [3,3], orthorhombic), x' = x L'/L, full
+ *  - allegro_md_deform: affine remap of the unwrapped positions to cell_new (HOST fp64 [3,3]), x' = x L'/L (x' = x H^-1 H' when
+ *    either cell is triclinic: the fractional coordinates are kept), full
  *    list rebuild and force evaluation.  A strain rate is a sequence of such increments between allegro_md_step calls.
  *  - allegro_set_state: checkpoint / resume — new pos, vel (DEVICE fp64 [N,3]) for the masses, species and cell given to
  *    allegro_md_init; rebuilds the list and the forces (NVE is deterministic given this state).

@@ -268,7 +268,7 @@ int allegro_energy_forces(void* h, const double* pos, const int32_t* species, in
   if (!m->nl.valid) { m->err = "allegro_energy_forces called before allegro_build_neighbors"; return ALLEGRO_ERR_NO_LIST; }
   if (N != m->nl.N) { m->err = "N differs from the neighbour list"; return ALLEGRO_ERR_INVALID; }
   for (int d = 0; d < 3; ++d)
-    if (cell[4 * d] != m->nl.L[d]) { m->err = "cell differs from the one the neighbour list was built with"; return ALLEGRO_ERR_INVALID; }
+    if (cell[3 * d] != m->nl.H[3 * d] || cell[3 * d + 1] != m->nl.H[3 * d + 1] || cell[3 * d + 2] != m->nl.H[3 * d + 2]) { m->err = "cell differs from the one the neighbour list was built with"; return ALLEGRO_ERR_INVALID; }
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   m->launches = 0;
   int rc = network_energy_forces(m, pos, species, N, E_out, F_out, E_atom_out, st);

@@ -14,7 +14,7 @@ struct ListView {
   const int64_t* rowptr;   // [N+1] list rows
   const uint64_t* keys;    // [E_list] packed (j, s)
   const int* revpos;       // [E_list]
-  double L[3];
+  double H[9];             // cell, rows = lattice vectors
 };
 
 __device__ __forceinline__ void decode_key(uint64_t key, int* j, int* sx, int* sy, int* sz) {
@@ -22,15 +22,20 @@ __device__ __forceinline__ void decode_key(uint64_t key, int* j, int* sx, int* s
   *sx = (int)((key >> 16) & 255) - 128; *sy = (int)((key >> 8) & 255) - 128; *sz = (int)(key & 255) - 128;
 }
 
-__device__ __forceinline__ double edge_d2(const double* __restrict__ pos, int64_t i, uint64_t key, const double* L,
+// Cartesian component c of the image shift s: (s_1 a_1c + s_2 a_2c) + s_3 a_3c, fp64, no FMA contraction (reading A27).  For a
+// diagonal H the two added products are exact zeros: the value is s_c L_c bit for bit, the expression of A16.
+__device__ __forceinline__ double image_shift(const double* H, int c, int sx, int sy, int sz) {
+  return __dadd_rn(__dadd_rn(__dmul_rn((double)sx, H[c]), __dmul_rn((double)sy, H[3 + c])), __dmul_rn((double)sz, H[6 + c]));
+}
+__device__ __forceinline__ double edge_d2(const double* __restrict__ pos, int64_t i, uint64_t key, const double* H,
                                           double* dx, double* dy, double* dz, int* jout) {
   int j, sx, sy, sz;
   decode_key(key, &j, &sx, &sy, &sz);
   *jout = j;
   // A16: same expression order as the list criterion, fp64, no FMA contraction
-  *dx = __dadd_rn(__dsub_rn(pos[3 * (int64_t)j], pos[3 * i]), __dmul_rn((double)sx, L[0]));
-  *dy = __dadd_rn(__dsub_rn(pos[3 * (int64_t)j + 1], pos[3 * i + 1]), __dmul_rn((double)sy, L[1]));
-  *dz = __dadd_rn(__dsub_rn(pos[3 * (int64_t)j + 2], pos[3 * i + 2]), __dmul_rn((double)sz, L[2]));
+  *dx = __dadd_rn(__dsub_rn(pos[3 * (int64_t)j], pos[3 * i]), image_shift(H, 0, sx, sy, sz));
+  *dy = __dadd_rn(__dsub_rn(pos[3 * (int64_t)j + 1], pos[3 * i + 1]), image_shift(H, 1, sx, sy, sz));
+  *dz = __dadd_rn(__dsub_rn(pos[3 * (int64_t)j + 2], pos[3 * i + 2]), image_shift(H, 2, sx, sy, sz));
   return __dadd_rn(__dadd_rn(__dmul_rn(*dx, *dx), __dmul_rn(*dy, *dy)), __dmul_rn(*dz, *dz));
 }
 
@@ -68,7 +73,7 @@ __global__ void k_active(const double* __restrict__ pos, const int* __restrict__
     double dx = 0, dy = 0, dz = 0, d2 = 0;
     int j = 0;
     if (k < e) {
-      d2 = edge_d2(pos, a, lv.keys[k], lv.L, &dx, &dy, &dz, &j);
+      d2 = edge_d2(pos, a, lv.keys[k], lv.H, &dx, &dy, &dz, &j);
       act = d2 < rc2;
     }
     const unsigned bal = __ballot_sync(0xffffffffu, act);
@@ -412,7 +417,7 @@ __global__ void __launch_bounds__(256) k_virial_partial(ListView lv, const doubl
   for (int64_t i = (int64_t)blockIdx.x * 8 + warp; i < N; i += (int64_t)gridDim.x * 8) {
     for (int64_t k = lv.rowptr[i] + lane; k < lv.rowptr[i + 1]; k += 32) {
       double d[3]; int j;
-      edge_d2(pos, i, lv.keys[k], lv.L, &d[0], &d[1], &d[2], &j);
+      edge_d2(pos, i, lv.keys[k], lv.H, &d[0], &d[1], &d[2], &j);
       const double g[3] = {(double)g_list[3 * k], (double)g_list[3 * k + 1], (double)g_list[3 * k + 2]};
 #pragma unroll
       for (int a = 0; a < 3; ++a)

@@ -59,6 +59,16 @@ __global__ void k_scale_pos(double* __restrict__ pos, int64_t N, double sx, doub
   pos[idx] *= (d == 0 ? sx : (d == 1 ? sy : sz));
 }
 
+// general cell: x' = x A with A = H^-1 H' (fractional coordinates kept), (x_0 A_0b + x_1 A_1b) + x_2 A_2b
+struct Affine { double A[9]; };
+__global__ void k_affine_pos(double* __restrict__ pos, int64_t N, Affine af) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const double x = pos[3 * i], y = pos[3 * i + 1], z = pos[3 * i + 2];
+#pragma unroll
+  for (int b = 0; b < 3; ++b) pos[3 * i + b] = __dadd_rn(__dadd_rn(__dmul_rn(x, af.A[b]), __dmul_rn(y, af.A[3 + b])), __dmul_rn(z, af.A[6 + b]));
+}
+
 __global__ void k_clear_flag(int* flags, int which) { flags[which] = 0; }
 
 __global__ void k_kinetic_partial(const double* __restrict__ vel, const double* __restrict__ mass, int64_t N, double* __restrict__ partial) {
@@ -262,18 +272,28 @@ int md_step(Model* m, double dt, int64_t n_steps, const double* nvt, cudaStream_
   return 0;
 }
 
-// A26: affine remap of the MD state to a new orthorhombic cell (x' = x L'/L), full list rebuild, forces re-evaluated.
+// A26: affine remap of the MD state to a new cell (x' = x L'/L; x' = x H^-1 H' when either cell is not orthorhombic), full list
+// rebuild, forces re-evaluated.
 int md_deform(Model* m, const double* cell_new, cudaStream_t st) {
   const int64_t N = m->nl.N;
+  bool diag = true;
   for (int a = 0; a < 3; ++a)
     for (int b = 0; b < 3; ++b)
-      if (a != b && cell_new[3 * a + b] != 0.0) { m->err = "non-orthorhombic cell (triclinic cells are not supported)"; return ALLEGRO_ERR_UNSUPPORTED; }
-  double sc[3];
-  for (int d = 0; d < 3; ++d) {
-    if (!(cell_new[4 * d] > 0.0)) { m->err = "cell lengths must be positive"; return ALLEGRO_ERR_INVALID; }
-    sc[d] = cell_new[4 * d] / m->md_cell[4 * d];
+      if (a != b && (cell_new[3 * a + b] != 0.0 || m->md_cell[3 * a + b] != 0.0)) diag = false;
+  if (diag) {
+    double sc[3];
+    for (int d = 0; d < 3; ++d) {
+      if (!(cell_new[4 * d] > 0.0)) { m->err = "cell lengths must be positive"; return ALLEGRO_ERR_INVALID; }
+      sc[d] = cell_new[4 * d] / m->md_cell[4 * d];
+    }
+    if (N > 0) k_scale_pos<<<(unsigned)((3 * N + 255) / 256), 256, 0, st>>>(m->md_pos.as<double>(), N, sc[0], sc[1], sc[2]);
+  } else {
+    const double* Hi = m->nl.Hinv;                      // inverse of the current cell (the list was built with it)
+    Affine af;
+    for (int a = 0; a < 3; ++a)
+      for (int b = 0; b < 3; ++b) af.A[3 * a + b] = (Hi[3 * a] * cell_new[b] + Hi[3 * a + 1] * cell_new[3 + b]) + Hi[3 * a + 2] * cell_new[6 + b];
+    if (N > 0) k_affine_pos<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(m->md_pos.as<double>(), N, af);
   }
-  if (N > 0) k_scale_pos<<<(unsigned)((3 * N + 255) / 256), 256, 0, st>>>(m->md_pos.as<double>(), N, sc[0], sc[1], sc[2]);
   for (int k = 0; k < 9; ++k) m->md_cell[k] = cell_new[k];
   md_graph_reset(m);
   if (int rc = nl_build(m, m->md_pos.as<double>(), N, m->md_cell, m->nl.cutoff, m->nl.skin, false, st)) return rc;

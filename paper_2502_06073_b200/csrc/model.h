@@ -34,7 +34,9 @@ struct CgDev {           // one tensor-product layer's tables on the device
 struct NeighborList {
   bool valid = false;
   int64_t N = 0;
-  double L[3] = {0, 0, 0};
+  double H[9] = {0};         // cell, rows = lattice vectors a_1, a_2, a_3 (reading A27); diagonal for an orthorhombic box
+  double Hinv[9] = {0};      // fractional coordinates f = x Hinv
+  bool ortho = true;
   double cutoff = 0, skin = 0;
   int nc[3] = {1, 1, 1};
   int64_t E_list = 0, cap = 0;

@@ -7,6 +7,7 @@
 // Every kernel can run "conditionally": it returns at once when flags[FLAG_REBUILD] == 0, so that the MD
 // loop can enqueue a rebuild without a host round trip.
 #include <algorithm>
+#include <cmath>
 #include <cstdio>
 
 #include "model.h"
@@ -130,9 +131,16 @@ __device__ __forceinline__ uint64_t make_key(int j, int sx, int sy, int sz) {
   return ((uint64_t)(uint32_t)j << 24) | ((uint64_t)(sx + 128) << 16) | ((uint64_t)(sy + 128) << 8) | (uint64_t)(sz + 128);
 }
 
+// as image_shift of edge_kernels.cuh (the two must stay the same expression)
+__device__ __forceinline__ double nl_image_shift(const double* H, int c, int sx, int sy, int sz) {
+  return __dadd_rn(__dadd_rn(__dmul_rn((double)sx, H[c]), __dmul_rn((double)sy, H[3 + c])), __dmul_rn((double)sz, H[6 + c]));
+}
+
 struct Grid {
-  double L[3], h[3];
+  double H[9], Hinv[9];    // cell (rows = lattice vectors) and its inverse: fractional coordinates f = x Hinv
+  double h[3];             // orthorhombic cell: bin width per axis
   int nc[3];
+  int ortho;
 };
 
 __global__ void k_bin_count(const double* __restrict__ pos, int64_t N, Grid g, int* __restrict__ img, int* __restrict__ cell_of,
@@ -141,15 +149,29 @@ __global__ void k_bin_count(const double* __restrict__ pos, int64_t N, Grid g, i
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= N) return;
   int c[3];
+  if (g.ortho) {
 #pragma unroll
-  for (int d = 0; d < 3; ++d) {
-    double x = pos[3 * i + d];
-    double w = floor(x / g.L[d]);
-    double xt = x - w * g.L[d];
-    int ci = (int)(xt / g.h[d]);
-    ci = max(0, min(ci, g.nc[d] - 1));
-    c[d] = ci;
-    img[3 * i + d] = (int)w;
+    for (int d = 0; d < 3; ++d) {
+      double x = pos[3 * i + d];
+      double w = floor(x / g.H[4 * d]);
+      double xt = x - w * g.H[4 * d];
+      int ci = (int)(xt / g.h[d]);
+      ci = max(0, min(ci, g.nc[d] - 1));
+      c[d] = ci;
+      img[3 * i + d] = (int)w;
+    }
+  } else {
+    // general cell (A27): bins in fractional coordinates; every point within R of x has |delta f_d| <= R / width_d <= 1 / nc_d
+    const double x = pos[3 * i], y = pos[3 * i + 1], z = pos[3 * i + 2];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      const double f = x * g.Hinv[d] + y * g.Hinv[3 + d] + z * g.Hinv[6 + d];
+      const double w = floor(f);
+      int ci = (int)((f - w) * (double)g.nc[d]);
+      ci = max(0, min(ci, g.nc[d] - 1));
+      c[d] = ci;
+      img[3 * i + d] = (int)w;
+    }
   }
   int cid = (c[0] * g.nc[1] + c[1]) * g.nc[2] + c[2];
   cell_of[i] = cid;
@@ -199,10 +221,10 @@ __global__ void k_nbr_pass(const double* __restrict__ pos, int64_t N, Grid g, do
           if (k < e) {
             j = sorted[k];
             sx = ix + wix - img[3 * j]; sy = iy + wiy - img[3 * j + 1]; sz = iz + wiz - img[3 * j + 2];
-            // A16: dx = (x_j - x_i) + s_x L_x, d2 = dx*dx + dy*dy + dz*dz, all fp64, no FMA contraction
-            double dx = __dadd_rn(__dsub_rn(pos[3 * j], xi), __dmul_rn((double)sx, g.L[0]));
-            double dy = __dadd_rn(__dsub_rn(pos[3 * j + 1], yi), __dmul_rn((double)sy, g.L[1]));
-            double dz = __dadd_rn(__dsub_rn(pos[3 * j + 2], zi), __dmul_rn((double)sz, g.L[2]));
+            // A16 / A27: dx = (x_j - x_i) + (s_1 a_1x + s_2 a_2x + s_3 a_3x), d2 = dx*dx + dy*dy + dz*dz, all fp64, no FMA contraction
+            double dx = __dadd_rn(__dsub_rn(pos[3 * j], xi), nl_image_shift(g.H, 0, sx, sy, sz));
+            double dy = __dadd_rn(__dsub_rn(pos[3 * j + 1], yi), nl_image_shift(g.H, 1, sx, sy, sz));
+            double dz = __dadd_rn(__dsub_rn(pos[3 * j + 2], zi), nl_image_shift(g.H, 2, sx, sy, sz));
             double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
             ok = (d2 < R2) && !(j == (int)i && sx == 0 && sy == 0 && sz == 0);
           }
@@ -300,14 +322,26 @@ int nl_build(Model* m, const double* pos, int64_t N, const double* cell, double 
   int* flags = m->flags.as<int>();
   const double R = cutoff + skin;
   if (!conditional) {
+    // cell: rows = lattice vectors (A27).  Perpendicular widths w_d = 1 / |column d of H^-1| (= L_d for an orthorhombic box)
+    nl.ortho = true;
     for (int a = 0; a < 3; ++a)
-      for (int b = 0; b < 3; ++b)
-        if (a != b && cell[3 * a + b] != 0.0) { m->err = "non-orthorhombic cell (triclinic cells are not supported)"; return ALLEGRO_ERR_UNSUPPORTED; }
+      for (int b = 0; b < 3; ++b) {
+        nl.H[3 * a + b] = cell[3 * a + b];
+        if (a != b && cell[3 * a + b] != 0.0) nl.ortho = false;
+      }
+    const double* H = nl.H;
+    const double det = H[0] * (H[4] * H[8] - H[5] * H[7]) - H[1] * (H[3] * H[8] - H[5] * H[6]) + H[2] * (H[3] * H[7] - H[4] * H[6]);
+    if (!(det > 0.0) || !std::isfinite(det)) { m->err = "cell must be right-handed with positive volume (cell lengths must be positive)"; return ALLEGRO_ERR_INVALID; }
+    const double cof[9] = {H[4] * H[8] - H[5] * H[7], H[2] * H[7] - H[1] * H[8], H[1] * H[5] - H[2] * H[4],
+                           H[5] * H[6] - H[3] * H[8], H[0] * H[8] - H[2] * H[6], H[2] * H[3] - H[0] * H[5],
+                           H[3] * H[7] - H[4] * H[6], H[1] * H[6] - H[0] * H[7], H[0] * H[4] - H[1] * H[3]};
+    for (int k = 0; k < 9; ++k) nl.Hinv[k] = cof[k] / det;
     for (int d = 0; d < 3; ++d) {
-      nl.L[d] = cell[4 * d];
-      if (!(nl.L[d] > 0.0)) { m->err = "cell lengths must be positive"; return ALLEGRO_ERR_INVALID; }
-      if (R > nl.L[d]) { m->err = "r_cut + skin exceeds the smallest box length (A17)"; return ALLEGRO_ERR_CUTOFF; }
-      int64_t c = (int64_t)floor(nl.L[d] / (R * (1.0 + 1e-9)));
+      const double width = nl.ortho ? H[4 * d]
+                                    : 1.0 / std::sqrt(nl.Hinv[d] * nl.Hinv[d] + nl.Hinv[3 + d] * nl.Hinv[3 + d] + nl.Hinv[6 + d] * nl.Hinv[6 + d]);
+      if (!(width > 0.0)) { m->err = "cell lengths must be positive"; return ALLEGRO_ERR_INVALID; }
+      if (R > width) { m->err = "r_cut + skin exceeds the smallest box length (perpendicular width of the cell; A17)"; return ALLEGRO_ERR_CUTOFF; }
+      int64_t c = (int64_t)floor(width / (R * (1.0 + 1e-9)));
       nl.nc[d] = (int)std::max<int64_t>(1, std::min<int64_t>(c, 1024));
     }
     // keep the number of cells bounded by ~N (tiny systems in huge boxes)
@@ -334,7 +368,9 @@ int nl_build(Model* m, const double* pos, int64_t N, const double* cell, double 
   }
   const int64_t ncell = (int64_t)nl.nc[0] * nl.nc[1] * nl.nc[2];
   Grid g;
-  for (int d = 0; d < 3; ++d) { g.L[d] = nl.L[d]; g.nc[d] = nl.nc[d]; g.h[d] = nl.L[d] / nl.nc[d]; }
+  for (int k = 0; k < 9; ++k) { g.H[k] = nl.H[k]; g.Hinv[k] = nl.Hinv[k]; }
+  for (int d = 0; d < 3; ++d) { g.nc[d] = nl.nc[d]; g.h[d] = nl.H[4 * d] / nl.nc[d]; }
+  g.ortho = nl.ortho ? 1 : 0;
   const int T = 256;
   const unsigned gridN = (unsigned)((N + T - 1) / T), gridW = (unsigned)((N * 32 + T - 1) / T);
   if (N == 0) {

@@ -11,6 +11,12 @@
 
 namespace allegro {
 
+static ListView list_view(const NeighborList& nl) {
+  ListView lv{nl.rowptr.as<int64_t>(), nl.keys.as<uint64_t>(), nl.revpos.as<int>(), {}};
+  for (int k = 0; k < 9; ++k) lv.H[k] = nl.H[k];
+  return lv;
+}
+
 namespace {
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 }
@@ -154,7 +160,7 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
   const int n = hp.n_channels, NL = hp.n_layers, D = P.D, nsc = P.n_sc, dsh = P.d_sh, S = hp.n_species, Nb = hp.n_bessel;
   const int64_t na = a1 - a0;
   const float inv_sqrt_navg = (float)(1.0 / std::sqrt(hp.avg_num_neighbors));
-  ListView lv{nl.rowptr.as<int64_t>(), nl.keys.as<uint64_t>(), nl.revpos.as<int>(), {nl.L[0], nl.L[1], nl.L[2]}};
+  const ListView lv = list_view(nl);
   const int T = 256;
   const unsigned gridWA = (unsigned)((na * 32 + T - 1) / T);
   // ---- active edges of the chunk
@@ -505,7 +511,7 @@ int network_energy_forces(Model* m, const double* pos, const int32_t* species, i
     const int64_t a1 = std::min(n_owned, a0 + atoms_per);
     if (int rc = run_chunk(m, pos, species, a0, a1, m->ws.cap_edges, st)) return rc;
   }
-  ListView lv{nl.rowptr.as<int64_t>(), nl.keys.as<uint64_t>(), nl.revpos.as<int>(), {nl.L[0], nl.L[1], nl.L[2]}};
+  const ListView lv = list_view(nl);
   if (N > 0) {
     prof_begin(m, st, KC_GATHER, 0);
     k_force_gather<<<(unsigned)((N * 32 + T - 1) / T), T, 0, st>>>(lv, N, m->g_list.as<float>(), F_out, flags);
@@ -529,7 +535,7 @@ int network_virial(Model* m, const double* pos, double* W_out, cudaStream_t st) 
   const int64_t N = nl.N;
   const int nb = (int)std::max<int64_t>(1, std::min<int64_t>(1024, (N + 7) / 8));
   if (int rc = ensure(m, &m->vir_partial, sizeof(double) * 9 * 1024)) return rc;
-  ListView lv{nl.rowptr.as<int64_t>(), nl.keys.as<uint64_t>(), nl.revpos.as<int>(), {nl.L[0], nl.L[1], nl.L[2]}};
+  const ListView lv = list_view(nl);
   if (N == 0) { cudaMemsetAsync(W_out, 0, sizeof(double) * 9, st); return 0; }
   k_virial_partial<<<nb, 256, 0, st>>>(lv, pos, N, m->g_list.as<float>(), m->vir_partial.as<double>());
   k_virial_final<<<1, 32, 0, st>>>(m->vir_partial.as<double>(), nb, W_out);

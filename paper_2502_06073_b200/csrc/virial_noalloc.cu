@@ -28,20 +28,24 @@ static_assert(VN_MAX_ATOMS == ALLEGRO_VIRIAL_NOALLOC_MAX_ATOMS, "include/allegro
 static __device__ __align__(256) double g_virial_scratch[(size_t)VN_MAX_BLOCKS * 9];
 
 // list key: j << 24 | (sx + 128) << 16 | (sy + 128) << 8 | (sz + 128)
-__device__ __forceinline__ void vn_edge(const double* __restrict__ pos, int64_t i, uint64_t key, double Lx, double Ly, double Lz, double* d) {
+struct VnCell { double H[9]; };   // rows = lattice vectors
+
+__device__ __forceinline__ void vn_edge(const double* __restrict__ pos, int64_t i, uint64_t key, const VnCell& cl, double* d) {
   const int64_t j = (int64_t)(key >> 24);
-  const int sx = (int)((key >> 16) & 255) - 128, sy = (int)((key >> 8) & 255) - 128, sz = (int)(key & 255) - 128;
-  // A16: the expression of the list criterion, fp64, no FMA contraction
-  d[0] = __dadd_rn(__dsub_rn(pos[3 * j], pos[3 * i]), __dmul_rn((double)sx, Lx));
-  d[1] = __dadd_rn(__dsub_rn(pos[3 * j + 1], pos[3 * i + 1]), __dmul_rn((double)sy, Ly));
-  d[2] = __dadd_rn(__dsub_rn(pos[3 * j + 2], pos[3 * i + 2]), __dmul_rn((double)sz, Lz));
+  const double sx = (double)((int)((key >> 16) & 255) - 128), sy = (double)((int)((key >> 8) & 255) - 128), sz = (double)((int)(key & 255) - 128);
+  // A16 / A27: the expression of the list criterion, fp64, no FMA contraction
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    const double sh = __dadd_rn(__dadd_rn(__dmul_rn(sx, cl.H[c]), __dmul_rn(sy, cl.H[3 + c])), __dmul_rn(sz, cl.H[6 + c]));
+    d[c] = __dadd_rn(__dsub_rn(pos[3 * j + c], pos[3 * i + c]), sh);
+  }
 }
 
 // Block b covers atoms [256 b, 256 b + 256): warp w the 32 atoms from 256 b + 32 w, lanes stride over a list row.  Fixed-shape
 // fp64 reduction (lane tree, warp partials in shared memory, one block partial [9]): deterministic, no atomics.
 __global__ void __launch_bounds__(256) k_virial_partial_na(const int64_t* __restrict__ rowptr, const uint64_t* __restrict__ keys,
                                                            const float* __restrict__ g_list, const double* __restrict__ pos, int64_t N,
-                                                           double Lx, double Ly, double Lz, double* __restrict__ partial) {
+                                                           VnCell cl, double* __restrict__ partial) {
   __shared__ double sh[8][9];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   double w[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
@@ -50,7 +54,7 @@ __global__ void __launch_bounds__(256) k_virial_partial_na(const int64_t* __rest
   for (int64_t i = i0; i < i1; ++i) {
     for (int64_t k = rowptr[i] + lane; k < rowptr[i + 1]; k += 32) {
       double d[3];
-      vn_edge(pos, i, keys[k], Lx, Ly, Lz, d);
+      vn_edge(pos, i, keys[k], cl, d);
       const double g[3] = {(double)g_list[3 * k], (double)g_list[3 * k + 1], (double)g_list[3 * k + 2]};
 #pragma unroll
       for (int a = 0; a < 3; ++a)
@@ -132,9 +136,10 @@ extern "C" int allegro_virial_noalloc(void* h, const double* pos, double* W_out,
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   const double* p = pos ? pos : m->md_pos.as<double>();
   const int nb = (int)((N + VN_ATOMS_PER_BLOCK - 1) / VN_ATOMS_PER_BLOCK);
+  VnCell cl;
+  for (int k = 0; k < 9; ++k) cl.H[k] = m->nl.H[k];
   if (nb > 0)
-    k_virial_partial_na<<<nb, 256, 0, st>>>(m->nl.rowptr.as<int64_t>(), m->nl.keys.as<uint64_t>(), m->g_list.as<float>(), p, N, m->nl.L[0],
-                                            m->nl.L[1], m->nl.L[2], scratch);
+    k_virial_partial_na<<<nb, 256, 0, st>>>(m->nl.rowptr.as<int64_t>(), m->nl.keys.as<uint64_t>(), m->g_list.as<float>(), p, N, cl, scratch);
   k_virial_final_na<<<1, 288, 0, st>>>(scratch, nb, W_out);   // nb == 0 writes zeros
   m->launches += nb > 0 ? 2 : 1;
   const cudaError_t e = cudaGetLastError();

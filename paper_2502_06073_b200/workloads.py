@@ -37,7 +37,7 @@ class Workload:
     pos: np.ndarray            # [N,3] fp64, Angstrom, unwrapped
     species: np.ndarray        # [N] int32 index into the species embedding
     mass: np.ndarray           # [N] fp64 amu
-    cell: np.ndarray           # [3,3] fp64 row vectors (orthorhombic)
+    cell: np.ndarray           # [3,3] fp64, rows = lattice vectors
     hp: dict                   # network hyper-parameters (keys mirror allegro_hparams)
     skin: float
     dt_fs: float

@@ -92,10 +92,12 @@ def test_errors(lib):
     with pytest.raises(lib.AllegroError) as ei:
         g.build_neighbors(p, s, np.diag([3.0, 8.0, 8.0]), 4.0, 0.0)
     assert ei.value.code == -6                                 # r_c + skin > box (A17)
-    tri = w.cell.copy(); tri[1, 0] = 0.5
     with pytest.raises(lib.AllegroError) as ei:
-        g.build_neighbors(p, s, tri, 4.0, 0.0)
-    assert ei.value.code == -2                                 # triclinic
+        g.build_neighbors(p, s, np.array([[8.0, 0, 0], [7.5, 3.9, 0], [0, 0, 8.0]]), 4.0, 0.0)
+    assert ei.value.code == -6                                 # triclinic: r_c + skin > a perpendicular width
+    with pytest.raises(lib.AllegroError) as ei:
+        g.build_neighbors(p, s, -w.cell, 4.0, 0.0)
+    assert ei.value.code == -1                                 # left-handed cell
     g.build_neighbors(p, s, w.cell, 4.0, 0.3)
     p2 = p.clone(); p2[5, 0] += 0.2
     with pytest.raises(lib.AllegroError) as ei:
