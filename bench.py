@@ -203,13 +203,13 @@ def roofline_for(prof, stats, clocks, peaks, n_sm, n_atoms, ms_md_step):
     fp32_peak = n_sm * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     hbm = peaks.get("hbm_gbs", 6650.0)
     tot_ms = sum(v["ms"] for v in prof.values()) or 1.0
-    dom = max((k for k in prof if k != "tp_mix"), key=lambda k: prof[k]["ms"])
+    dom = max((k for k in prof if k not in ("tp_mix", "tp_mix16")), key=lambda k: prof[k]["ms"])
     E_act, E_list = stats["active_edges"], stats["list_edges"]
     chunks = max(1, stats.get("chunks", 1))
-    shares = {k: round(v["ms"] / tot_ms, 4) for k, v in prof.items() if v["launches"] and k != "tp_mix"}
+    shares = {k: round(v["ms"] / tot_ms, 4) for k, v in prof.items() if v["launches"] and k not in ("tp_mix", "tp_mix16")}
     names = {"gemm": "k_gemm_chain", "gemm_f16s": "k_gemm_f16s", "tp_fwd": "k_tp_fwd3 / k_tpo_fwd", "tp_bwd": "k_tp_bwd3 / k_tpo_bwd"}
     roof = {"kernel": names.get(dom, dom), "shares": shares}
-    flops = {k: prof[k]["work"] * E_act / chunks for k in ("gemm", "gemm_f16s", "tp_fwd", "tp_bwd", "tp_mix") if k in prof}
+    flops = {k: prof[k]["work"] * E_act / chunks for k in ("gemm", "gemm_f16s", "tp_fwd", "tp_bwd", "tp_mix", "tp_mix16") if k in prof}
     traffic, traffic_src = None, None
     try:
         tr = json.load(open(os.path.join(ROOT, "profiles", "r2_traffic.json")))
@@ -232,14 +232,14 @@ def roofline_for(prof, stats, clocks, peaks, n_sm, n_atoms, ms_md_step):
         roof.update({"bound": "hbm", "achieved": None, "peak": hbm, "unit": "GB/s", "frac": None, "traffic": traffic,
                      "peak_source": "MEASURED_PEAKS.json" if peaks else "fallback"})
     # ---- per MD step: t_roof = max(F_gemm / P_tc, F_alu / P_fp32, B_alg / BW_hbm)
-    t_tensor = ((flops.get("gemm", 0.0) + flops.get("tp_mix", 0.0)) / (peak_tf32x3 * 1e12) + flops.get("gemm_f16s", 0.0) / (peak_f16s * 1e12)) * 1e3
+    t_tensor = ((flops.get("gemm", 0.0) + flops.get("tp_mix", 0.0)) / (peak_tf32x3 * 1e12) + (flops.get("gemm_f16s", 0.0) + flops.get("tp_mix16", 0.0)) / (peak_f16s * 1e12)) * 1e3
     t_alu = (flops.get("tp_fwd", 0.0) + flops.get("tp_bwd", 0.0)) / (fp32_peak * 1e12) * 1e3
     b_alg = 52.0 * n_atoms + 8.0 * E_list + 96.0 * n_atoms
     t_hbm = b_alg / (hbm * 1e9) * 1e3
     t_roof = max(t_tensor, t_alu, t_hbm)
     roof["per_step"] = {"t_step_ms": ms_md_step, "t_roof_ms": t_roof, "frac": t_roof / ms_md_step,
                         "t_tensor_ms": t_tensor, "t_alu_ms": t_alu, "t_hbm_ms": t_hbm,
-                        "gemm_flop": flops.get("gemm", 0.0) + flops.get("gemm_f16s", 0.0) + flops.get("tp_mix", 0.0),
+                        "gemm_flop": flops.get("gemm", 0.0) + flops.get("gemm_f16s", 0.0) + flops.get("tp_mix", 0.0) + flops.get("tp_mix16", 0.0),
                         "alu_flop": flops.get("tp_fwd", 0.0) + flops.get("tp_bwd", 0.0), "algorithmic_bytes": b_alg,
                         "peaks": {"tensor_f16_split_tflops": peak_f16s, "tensor_tf32x3_tflops": peak_tf32x3, "fp32_tflops": fp32_peak,
                                   "hbm_gbs": hbm, "tensor_peak_kind": "burst" if at_max else "sustained"},

@@ -118,6 +118,11 @@ int allegro_md_deform(void* h, const double* cell_new, void* stream);
 int allegro_set_state(void* h, const double* pos, const double* vel, void* stream);
 int allegro_virial(void* h, const double* pos, double* W_out, void* stream);
 
+/* Test hook: on = 0 makes the many-channel networks (n = 64) run the forward tensor product and the channel mixing as separate
+ * kernels with the per-path products T in HBM (k_tpo_fwd + one GEMM per output irrep) instead of the fused kernel of tp_mix.cu
+ * (default, on = 1).  Same arithmetic, other summation order: tests compare the two. */
+int allegro_debug_set_fusion(void* h, int on);
+
 /* allegro_virial for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
  * cudaMalloc): same arguments, same quantity (the summation order of the fp64 reduction differs, so the last bits may), but
  *  - the call contains no cudaMalloc / cudaFree / allocating library routine and no stream synchronisation: two kernel launches
@@ -174,10 +179,11 @@ int allegro_get_stats(void* h, int64_t* stats);
 /* Per-kernel-class timing for bench.py's roofline line.  allegro_profile(h, 1) resets the counters and makes
  * every launch of the following calls bracketed by CUDA events on the launching stream; allegro_profile(h, 0)
  * stops it.  allegro_get_profile synchronises and returns, per class k (0 gemm, 1 tp_fwd, 2 tp_bwd, 3 gamma,
- * 4 gammabar, 5 active_edges, 6 edge_misc, 7 neighbor, 8 md, 9 force_gather, 10 gemm_f16s, 11 tp_mix; class 0 = the 3xTF32 kernels of
- * gemm_tc.cu, class 10 = the split-fp16 kernel of gemm_f16s.cu, class 11 carries only work: the channel-mixing flop that the
- * few-channel tensor-product kernels run on mma.sync inside classes 1-2): ms[k] total device time, launches[k], work[k] =
- * algorithmic flop per active edge summed over the class's launches (classes 0-2, 10, 11, else 0).
+ * 4 gammabar, 5 active_edges, 6 edge_misc, 7 neighbor, 8 md, 9 force_gather, 10 gemm_f16s, 11 tp_mix, 12 tp_mix16; class 0 = the
+ * 3xTF32 kernels of gemm_tc.cu, class 10 = the split-fp16 kernel of gemm_f16s.cu, classes 11 and 12 carry only work: the
+ * channel-mixing flop that tensor-product kernels timed in classes 1-2 run on tensor cores themselves (11: mma.sync 3xTF32 in the
+ * few-channel kernels, 12: tcgen05 split-fp16 in tp_mix.cu)): ms[k] total device time, launches[k], work[k] =
+ * algorithmic flop per active edge summed over the class's launches (classes 0-2, 10-12, else 0).
  * HOST arrays of max_classes entries; returns the number of classes.  Never enabled inside a timed throughput run. */
 int allegro_profile(void* h, int enable);
 int allegro_get_profile(void* h, double* ms, int64_t* launches, double* work, int max_classes);

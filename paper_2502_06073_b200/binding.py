@@ -24,14 +24,14 @@ ERR_NAMES = {0: "OK", -1: "INVALID", -2: "UNSUPPORTED", -3: "CUDA", -4: "STALE_L
              -7: "SPECIES", -8: "NO_LIST", -9: "ALLOC"}
 EXPORTS = ["allegro_weight_layout", "allegro_create", "allegro_destroy", "allegro_build_neighbors",
            "allegro_energy_forces", "allegro_md_init", "allegro_md_step", "allegro_md_step_nvt", "allegro_md_deform",
-           "allegro_set_state", "allegro_virial", "allegro_virial_noalloc", "allegro_debug_set_list_slack", "allegro_energy_forces_owned",
+           "allegro_set_state", "allegro_virial", "allegro_virial_noalloc", "allegro_debug_set_fusion", "allegro_debug_set_list_slack", "allegro_energy_forces_owned",
            "allegro_decomp_select", "allegro_decomp_scatter", "allegro_kick_drift", "allegro_get_state",
            "allegro_get_neighbors", "allegro_get_stats", "allegro_profile", "allegro_get_profile",
            "allegro_debug_coupling", "allegro_debug_num_paths", "allegro_debug_set_precision", "allegro_debug_gemm",
            "allegro_last_error"]
 VIRIAL_NOALLOC_MAX_ATOMS = 1048576   # ALLEGRO_VIRIAL_NOALLOC_MAX_ATOMS of include/allegro.h
 PROFILE_CLASSES = ["gemm", "tp_fwd", "tp_bwd", "gamma", "gammabar", "active_edges", "edge_misc", "neighbor", "md",
-                   "force_gather", "gemm_f16s", "tp_mix"]
+                   "force_gather", "gemm_f16s", "tp_mix", "tp_mix16"]
 
 
 class HParams(C.Structure):
@@ -62,6 +62,7 @@ _lib.allegro_md_deform.argtypes = [_vp, _vp, _vp]
 _lib.allegro_set_state.argtypes = [_vp, _vp, _vp, _vp]
 _lib.allegro_virial.argtypes = [_vp, _vp, _vp, _vp]
 _lib.allegro_virial_noalloc.argtypes = [_vp, _vp, _vp, _vp]
+_lib.allegro_debug_set_fusion.argtypes = [_vp, C.c_int]
 _lib.allegro_debug_set_list_slack.argtypes = [_vp, _dbl, _i64]
 _lib.allegro_energy_forces_owned.argtypes = [_vp, _vp, _vp, _i64, _vp, _i64, _vp, _vp, _vp, _vp]
 _lib.allegro_decomp_select.argtypes = [_vp, _vp, _vp, _i64, _vp, _vp, _vp, _dbl, _i64, _vp, _vp, _vp, _vp, _vp, _vp]
@@ -224,6 +225,9 @@ class Allegro:
         """allegro_virial_noalloc: writes the virial into W_out (torch CUDA fp64, 9 elements, the caller's buffer) on the current
         stream without allocating or synchronising; at most VIRIAL_NOALLOC_MAX_ATOMS atoms; calls that overlap on the GPU race."""
         self._check(_lib.allegro_virial_noalloc(self._h, _ptr(pos), _ptr(W_out), _stream()))
+
+    def debug_set_fusion(self, on: bool):
+        self._check(_lib.allegro_debug_set_fusion(self._h, int(bool(on))))
 
     def debug_set_list_slack(self, frac, extra):
         self._check(_lib.allegro_debug_set_list_slack(self._h, float(frac), int(extra)))

@@ -13,11 +13,13 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "liballegro_b200.so")
-SOURCES = ["plan.cpp", "neighbor.cu", "network.cu", "tp_kernels.cu", "tp3_fwd.cu", "tp3_bwd.cu", "gemm_tc.cu", "gemm_f16s.cu", "decomp.cu", "virial_noalloc.cu", "md.cu", "api.cu"]
+SOURCES = ["plan.cpp", "neighbor.cu", "network.cu", "tp_kernels.cu", "tp3_fwd.cu", "tp3_bwd.cu", "gemm_tc.cu", "gemm_f16s.cu", "decomp.cu", "virial_noalloc.cu", "tp_mix.cu", "md.cu", "api.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr", "-Xptxas", "-v" if os.environ.get("ALLEGRO_PTXAS_V") else "-O3"]
 if os.environ.get("ALLEGRO_F16S_TRACE"):   # developer build: gemm_f16s.cu prints the per-tile timeline of CTA 0 after every launch
     NVCC_FLAGS.append("-DF16S_TRACE")
+if os.environ.get("ALLEGRO_X_TRACE"):   # developer build: tp_mix.cu prints the wait times of CTA 0
+    NVCC_FLAGS.append("-DX_TRACE"); NVCC_FLAGS.append("-DX_FEWMMA") if os.environ.get("ALLEGRO_X_FEWMMA") else None
 if os.environ.get("ALLEGRO_F16S_DBGWAIT"):   # developer build: barrier waits time out and report their source line instead of trapping
     NVCC_FLAGS.append("-DF16S_DBGWAIT")
 

@@ -412,6 +412,12 @@ int allegro_virial(void* h, const double* pos, double* W_out, void* stream) {
   return ALLEGRO_OK;
 }
 
+int allegro_debug_set_fusion(void* h, int on) {
+  if (!h) return ALLEGRO_ERR_INVALID;
+  static_cast<Model*>(h)->use_tpmix = on != 0;
+  return ALLEGRO_OK;
+}
+
 int allegro_debug_set_list_slack(void* h, double frac, int64_t extra) {
   if (!h || frac < 0.0 || extra < 0) return ALLEGRO_ERR_INVALID;
   Model* m = static_cast<Model*>(h);

@@ -136,6 +136,7 @@ bool launch_gemm_chain(Model* m, const GemmArgs* stages, int n_stages, int64_t m
 
 // split-fp16 tcgen05 kernel for the wide linears (gemm_f16s.cu); false = shape / alignment outside what it takes
 bool launch_gemm_f16s(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st);
+const uint8_t* f16s_packed_weights(Model* m, const GemmArgs& a, cudaStream_t st, const float** out_scale);
 // species columns of the first two-body matrix, transposed once and cached: WgT[z][n] = Wg[n * ldwg + z], z < 2S (gemm_tc.cu)
 const float* transposed_species_columns(Model* m, const GemmArgs& a, cudaStream_t st);
 

@@ -587,6 +587,12 @@ uint8_t* packed_weights16(Model* m, const GemmArgs& a, cudaStream_t st, int* Npa
 
 }  // namespace
 
+// packed b_hi | b_lo | b_b stages of a weight matrix (cached per call site) and its 2^-s, for tp_mix.cu
+const uint8_t* f16s_packed_weights(Model* m, const GemmArgs& a, cudaStream_t st, const float** out_scale) {
+  int Npad = 0, Kpad = 0;
+  return packed_weights16(m, a, st, &Npad, &Kpad, out_scale);
+}
+
 // Returns false when the shape / alignment is outside what the kernel takes (the caller then uses k_gemm_tc).
 bool launch_gemm_f16s(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st) {
   const int K = a.K0 + a.K1;

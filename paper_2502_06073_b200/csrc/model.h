@@ -72,7 +72,7 @@ struct Workspace {       // per-chunk activations, sized for cap_edges active ed
 };
 
 // optional per-kernel-class timing with CUDA events on the launching stream (allegro_profile)
-enum { KC_GEMM = 0, KC_TP_FWD, KC_TP_BWD, KC_GAMMA, KC_GAMMABAR, KC_ACTIVE, KC_EDGE_MISC, KC_NEIGHBOR, KC_MD, KC_GATHER, KC_GEMM16, KC_TP_MIX, KC_COUNT };
+enum { KC_GEMM = 0, KC_TP_FWD, KC_TP_BWD, KC_GAMMA, KC_GAMMABAR, KC_ACTIVE, KC_EDGE_MISC, KC_NEIGHBOR, KC_MD, KC_GATHER, KC_GEMM16, KC_TP_MIX, KC_TP_MIX16, KC_COUNT };
 struct Prof {
   bool on = false;
   std::vector<cudaEvent_t> ev;      // pairs
@@ -91,6 +91,7 @@ struct Model {
   int num_sms = 148;
   bool use_tc = true;              // dense linears on tcgen05
   bool use_chain = true;           // MLP chains in one kernel (gemm_tc.cu k_gemm_chain) where the widths fit
+  bool use_tpmix = true;           // n = 64: forward tensor product + channel mixing in one kernel (tp_mix.cu)
   bool use_big = false;            // many-channel tensor product: T buffers + tcgen05 channel mixing (tp_big.cuh)
   bool use_tp3 = true;             // few-channel tensor-product kernels (tp3.cuh) where the channel count is 8, 16 or 32, else tp.cuh
   float* d_w = nullptr;            // weight blob

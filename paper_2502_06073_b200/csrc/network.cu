@@ -262,6 +262,12 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
       prof_begin(m, st, KC_TP_FWD, tp_work(P, L, false, &mixf));
       if (m->prof.on && !(m->use_big && tpbig_supported(tp))) m->prof.work[KC_TP_MIX] += mixf;
       if (m->use_big && tpbig_supported(tp)) {
+        // many channels, n = 64: tensor product and channel mixing in one kernel (tp_mix.cu), T stays on chip
+        if (m->use_tpmix && launch_tpmix_fwd(m, m->tp_sig[L - 1], st, tp, io)) {
+          if (m->prof.on) m->prof.work[KC_TP_MIX16] += mixf;
+          prof_end(m, st);
+          prof_begin(m, st, KC_TP_FWD, 0);
+        } else {
         // many channels: tensor product to per-irrep T buffers, channel mixing as tcgen05 GEMMs written straight into V^L
         TpBig big{};
         size_t off = 0;
@@ -278,6 +284,7 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
           launch_gemm(m, gm, m_cap * tp.out_d3[o], st);
         }
         prof_begin(m, st, KC_TP_FWD, 0);
+        }
       } else if (tp3_supported(tp) && m->use_tp3) {
         const size_t sm3 = tp3_smem_bytes(tp, false);
         const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(3, (227 * 1024) / (sm3 + 2048)));

@@ -89,6 +89,7 @@ void launch_tp3(int sig, bool backward, int grid, cudaStream_t st, const TpLayer
 struct TpBig;
 bool tpbig_supported(const TpLayerDev& tp);
 size_t tpbig_floats_per_edge(const TpLayerDev& tp);
+bool launch_tpmix_fwd(Model* m, int sig, cudaStream_t st, const TpLayerDev& tp, const TpIo& io);   // tp_mix.cu
 void launch_tpo(int sig, bool backward, int64_t m_cap, cudaStream_t st, const TpLayerDev& tp, const TpIo& io, const TpBig& big);
 
 constexpr int TP_MAXMT = 2;   // 4x4 micro-tiles per thread (forward): TE * d3 * n <= 8192

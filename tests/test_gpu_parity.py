@@ -199,3 +199,23 @@ def test_md_skin_rebuilds_match_oracle(lib):
     assert np.abs(p - ref["pos"]).max() <= 1e-4
     # list after MD equals the oracle's list at the last rebuild positions? -> at least symmetric & consistent E
     assert abs(Ep - ref["E_pot"]) <= E_RTOL * abs(ref["E_pot"])
+
+
+# ------------------------------------------------------------------------------------------------ fused forward layer (tp_mix.cu)
+@pytest.mark.parametrize("net", [(2, 2, 64, [40, 32]), (3, 3, 64, [36, 28])])
+def test_fused_tensor_product_and_mixing_equals_the_unfused_path(lib, net):
+    """n = 64: k_tpmix_fwd (T on chip) against k_tpo_fwd + per-irrep GEMMs (T in HBM), and both against the oracle."""
+    lmax, NL, n, lat = net
+    hp = WL.hparams(3, lmax, NL, n, [24, lat[-1]], lat, [12], 4.0, 18.0, n_bessel=6)
+    g, o = _model(lib, hp, 77)
+    pos, sp, cell = WL.small_periodic(5, 2.2, 0.4, 3, seed=31)         # 125 atoms: several 16-edge tiles and a ragged one
+    Eo, Fo, Eao = o.energy_forces(pos, sp, cell, O.neighbors_bruteforce(pos, cell, 4.0))
+    out = {}
+    for fused in (True, False):
+        g.debug_set_fusion(fused)
+        E, F, Ea = g.compute(pos, sp, cell, skin=0.3, want_atom=True)
+        _check_ef(E, F, Eo, Fo, Ea, Eao)
+        out[fused] = (E, F, Ea)
+    rms = math.sqrt((Fo ** 2).mean())
+    assert abs(out[True][0] - out[False][0]) <= 2e-7 * abs(Eo)
+    assert np.abs(out[True][1] - out[False][1]).max() <= 5e-6 * rms
