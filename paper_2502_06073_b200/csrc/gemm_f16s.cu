@@ -195,7 +195,7 @@ __global__ void __launch_bounds__(F_T, 1) k_gemm_f16s(const __grid_constant__ FA
                                                        const __grid_constant__ CUtensorMap tmA1, const __grid_constant__ CUtensorMap tmC,
                                                        const __grid_constant__ CUtensorMap tmC2) {
   extern __shared__ uint8_t smem_dyn[];
-  __shared__ __align__(8) uint64_t raw_full[F_S], cvt_full[F_S], b_full[F_S], mma_done[F_S];
+  __shared__ __align__(8) uint64_t raw_full[F_S], cvt_full[F_S], mma_done[F_S];
   __shared__ __align__(8) uint64_t acc_full[2], acc_empty[2];
   __shared__ uint32_t tmem_base_s;
   const GemmArgs& a = fa.a;
@@ -215,8 +215,8 @@ __global__ void __launch_bounds__(F_T, 1) k_gemm_f16s(const __grid_constant__ FA
   }
   if (tid == 32) {
     for (int s = 0; s < F_S; ++s) {
-      mbar_init(&raw_full[s], 1); mbar_init(&cvt_full[s], F_CVT);
-      mbar_init(&b_full[s], 1); mbar_init(&mma_done[s], 1);
+      mbar_init(&raw_full[s], 1); mbar_init(&cvt_full[s], F_CVT + 1);   // the converter warps + the weight copy: one wait per stage for the issuing thread
+      mbar_init(&mma_done[s], 1);
     }
     for (int b = 0; b < 2; ++b) { mbar_init(&acc_full[b], 1); mbar_init(&acc_empty[b], F_EPI); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -266,7 +266,7 @@ __global__ void __launch_bounds__(F_T, 1) k_gemm_f16s(const __grid_constant__ FA
           if ((int)(it & 1) != w) continue;
           const uint32_t slot = it % F_S, ph = (it / F_S) & 1;
           TR_WAIT(0, mbar_wait_b(&mma_done[slot], ph ^ 1))
-          bulk_g2s(smem + (size_t)slot * F_STAGE_BYTES + F_OFF_B, tb + (size_t)ks * Nt * (F_KS * 6), (uint32_t)Nt * (F_KS * 6), &b_full[slot]);
+          bulk_g2s(smem + (size_t)slot * F_STAGE_BYTES + F_OFF_B, tb + (size_t)ks * Nt * (F_KS * 6), (uint32_t)Nt * (F_KS * 6), &cvt_full[slot]);
         }
       }
       if (w == 0) TR_FLUSH(16)
@@ -288,7 +288,6 @@ __global__ void __launch_bounds__(F_T, 1) k_gemm_f16s(const __grid_constant__ FA
         for (int ks = 0; ks < nk; ++ks, ++it) {
           const uint32_t slot = it % F_S, ph = (it / F_S) & 1;
           TR_WAIT(1, mbar_wait_b(&cvt_full[slot], ph))
-          TR_WAIT(2, mbar_wait_b(&b_full[slot], ph))
           asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
           const uint32_t sbase = smem_u32(smem + (size_t)slot * F_STAGE_BYTES);
           const uint32_t sa_hi = sbase, sa_lo = sa_hi + F_CVT_BYTES;
