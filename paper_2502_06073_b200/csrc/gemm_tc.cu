@@ -281,10 +281,10 @@ void launch_gemm_tc(Model* m, const GemmArgs& a, int64_t m_cap, cudaStream_t st)
   int tmem_cols = 32;
   while (tmem_cols < Nt) tmem_cols *= 2;
   const size_t smem = 2 * (size_t)(2 * TC_M * TC_KC * 4 + 2 * Nt * TC_KC * 4);
-  static bool attr_set = false;
-  if (!attr_set) {
+  static int attr_dev = -1;   // the attribute is per device
+  if (attr_dev != m->device) {
     cudaFuncSetAttribute(k_gemm_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * (2 * TC_M * TC_KC * 4 + 2 * TC_NMAX * TC_KC * 4));
-    attr_set = true;
+    attr_dev = m->device;
   }
   auto al = [](const void* p) { return ((uintptr_t)p & 15) == 0; };
   int vec_ok = (a.N % 4 == 0) && (a.ldc % 4 == 0) && al(a.C);
@@ -683,6 +683,8 @@ bool launch_gemm_chain(Model* m, const GemmArgs* stages, int n_stages, int64_t m
     const int K = a.K0 + a.K1;
     if (K > CH_KMAX || a.N > CH_NMAX) return false;
     if (s > 0 && (a.K1 != 0 || a.K0 != stages[s - 1].N)) return false;
+    // a chained stage reads the previous stage's output from TMEM: it must BE that output (C, or C2 of a two-output epilogue)
+    if (s > 0 && a.A0 != stages[s - 1].C && a.A0 != stages[s - 1].C2) return false;
     bool vec_ok = (a.N % 4 == 0) && (a.ldc % 4 == 0) && al(a.C);
     if (a.C2) vec_ok = vec_ok && (a.ldc2 % 4 == 0) && al(a.C2);
     if (a.aux) vec_ok = vec_ok && (a.ldaux % 4 == 0) && al(a.aux);
@@ -710,8 +712,8 @@ bool launch_gemm_chain(Model* m, const GemmArgs* stages, int n_stages, int64_t m
   (void)nmax;
   // A staging 32 KB + CH_NB weight slots 48 KB + one prefetch tile per compute warp 16 KB = 96 KB: two CTAs per SM
   const size_t smem = (size_t)(2 * 2 * TC_M * TC_KC + CH_NB * 2 * CH_NMAX * TC_KC + 8 * 32 * WT_LD) * sizeof(float);
-  static bool attr_set = false;
-  if (!attr_set) { cudaFuncSetAttribute(k_gemm_chain, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_set = true; }
+  static int attr_dev = -1;   // the attribute is per device
+  if (attr_dev != m->device) { cudaFuncSetAttribute(k_gemm_chain, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_dev = m->device; }
   prof_begin(m, st, KC_GEMM, work);
   k_gemm_chain<<<(unsigned)((m_cap + TC_M - 1) / TC_M), CH_T, smem, st>>>(ca);
   prof_end(m, st);

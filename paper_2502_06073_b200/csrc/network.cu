@@ -182,19 +182,24 @@ static int run_chunk(Model* m, const double* pos, const int32_t* species, int64_
 
   // Dependent linears are collected and launched as one chained kernel where the shapes allow (gemm_tc.cu)
   std::vector<GemmArgs> ch;
-  auto flush = [&]() {   // returns true when every stage went through the chained kernel (fused row dots included)
-    bool all = true;
+  // Returns true when every stage that carries a fused row dot went through the chained kernel (which computes it); false when
+  // such a stage fell back to a single-linear launch, which does not — the caller then runs the dot as its own kernel.  (Groups
+  // are decided one by one: a fallback of a group WITHOUT a dot must not make the caller add the dot a second time.)
+  auto flush = [&]() {
+    bool dots_fused = true;
     size_t i = 0;
     while (i < ch.size()) {
       const size_t cnt = std::min<size_t>(4, ch.size() - i);
       if (!launch_gemm_chain(m, ch.data() + i, (int)cnt, m_cap, st)) {
-        all = false;
-        for (size_t k = i; k < i + cnt; ++k) launch_gemm(m, ch[k], m_cap, st);
+        for (size_t k = i; k < i + cnt; ++k) {
+          if (ch[k].dot_out) dots_fused = false;
+          launch_gemm(m, ch[k], m_cap, st);
+        }
       }
       i += cnt;
     }
     ch.clear();
-    return all;
+    return dots_fused;
   };
   // ---- F4: two-body MLP.  First layer = gather of the two one-hot columns + N_b-wide mat-vec.
   GemmArgs g;

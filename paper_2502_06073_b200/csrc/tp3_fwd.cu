@@ -7,8 +7,10 @@ namespace allegro {
 
 template <int SIG, int NCH>
 static void launch_t(int grid, size_t smem, cudaStream_t st, const TpLayerDev& tp, const TpIo& io) {
-  static bool attr = false;
-  if (!attr) { cudaFuncSetAttribute(k_tp_fwd3<SIG, NCH>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); attr = true; }
+  static int attr_dev = -1;   // the attribute is per device
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (attr_dev != dev) { cudaFuncSetAttribute(k_tp_fwd3<SIG, NCH>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); attr_dev = dev; }
   k_tp_fwd3<SIG, NCH><<<grid, 256, smem, st>>>(tp, io);
 }
 template <int SIG>

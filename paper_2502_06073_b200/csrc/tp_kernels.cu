@@ -8,11 +8,13 @@ namespace allegro {
 
 // launch the generated instantiation of the tensor-product kernels for layer signature `sig`
 void launch_tp_fwd(int sig, dim3 grid, size_t smem, cudaStream_t st, const TpLayerDev& tp, const TpIo& io, int TE, int PC) {
-  static bool attr[tpgen::N_SIGS] = {false};
+  static int attr[tpgen::N_SIGS] = {0};   // device ordinal + 1 the attribute was last set on (it is per device)
+  int dev = 0;
+  cudaGetDevice(&dev);
   switch (sig) {
 #define X(I)                                                                                                        \
   case I:                                                                                                           \
-    if (!attr[I]) { cudaFuncSetAttribute(k_tp_fwd<I>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); attr[I] = true; } \
+    if (attr[I] != dev + 1) { cudaFuncSetAttribute(k_tp_fwd<I>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); attr[I] = dev + 1; } \
     k_tp_fwd<I><<<grid, TP_T, smem, st>>>(tp, io, TE, PC);                                                            \
     break;
     TPGEN_FOR_EACH_SIG(X)
@@ -21,11 +23,13 @@ void launch_tp_fwd(int sig, dim3 grid, size_t smem, cudaStream_t st, const TpLay
   }
 }
 void launch_tp_bwd(int sig, dim3 grid, size_t smem, cudaStream_t st, const TpLayerDev& tp, const TpIo& io, int TE, int d3max, int PC) {
-  static bool attr[tpgen::N_SIGS] = {false};
+  static int attr[tpgen::N_SIGS] = {0};   // device ordinal + 1 the attribute was last set on (it is per device)
+  int dev = 0;
+  cudaGetDevice(&dev);
   switch (sig) {
 #define X(I)                                                                                                        \
   case I:                                                                                                           \
-    if (!attr[I]) { cudaFuncSetAttribute(k_tp_bwd<I>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024); attr[I] = true; } \
+    if (attr[I] != dev + 1) { cudaFuncSetAttribute(k_tp_bwd<I>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024); attr[I] = dev + 1; } \
     k_tp_bwd<I><<<grid, TP_T, smem, st>>>(tp, io, TE, d3max, PC);                                                     \
     break;
     TPGEN_FOR_EACH_SIG(X)
