@@ -156,7 +156,7 @@ class ClockSampler:
             out, _ = self.p.communicate(timeout=5)
         except Exception:
             self.p.kill(); out = ""
-        sm, mx, reasons = [], [], set()
+        sm, mx, pw, reasons = [], [], [], set()
         for ln in out.strip().splitlines():
             f = [x.strip() for x in ln.split(",")]
             if len(f) < 9:
@@ -165,11 +165,15 @@ class ClockSampler:
                 sm.append(float(f[1])); mx.append(float(f[2]))
             except ValueError:
                 continue
+            try:
+                pw.append(float(f[3]))
+            except ValueError:
+                pass
             for name, v in zip(["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"], f[5:9]):
                 if v.lower().startswith("active"):
                     reasons.add(name)
         return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+                "reasons": sorted(reasons), "samples": len(sm), "power_w": statistics.median(pw) if pw else None}
 
 
 def max_over_ranks(values, world, device="cpu"):

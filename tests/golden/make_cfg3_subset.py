@@ -16,7 +16,7 @@ sys.path.insert(0, ROOT)
 from oracle import allegro_oracle as O                      # noqa: E402
 from paper_2502_06073_b200 import workloads as WL           # noqa: E402
 
-N_TARGETS, N_LIST_ROWS, SEED = 16, 64, 13
+N_TARGETS, N_LIST_ROWS, SEED = 64, 128, 13
 
 
 def main():
