@@ -117,10 +117,11 @@ def test_energy_forces_cfg0(lib):
     E, F, Ea = g.compute(w.pos, w.species, w.cell, skin=w.skin, want_atom=True)
     Eo, Fo, Eao = o.energy_forces(w.pos, w.species, w.cell, O.neighbors_bruteforce(w.pos, w.cell, w.hp["r_cut"]))
     _check_ef(E, F, Eo, Fo, Ea, Eao)
-    assert g.get_stats()["active_edges"] == 1880 or True
+    assert g.get_stats()["active_edges"] == int(O.neighbors_bruteforce(w.pos, w.cell, w.hp["r_cut"])[0][-1])
 
 
-@pytest.mark.parametrize("net", [(1, 1, 8), (2, 2, 8), (3, 3, 8), (3, 2, 4), (2, 3, 12), (3, 3, 16), (2, 2, 64), (3, 3, 64)])
+@pytest.mark.parametrize("net", [(1, 1, 8), (2, 2, 8), (3, 3, 8), (3, 2, 4), (2, 3, 12), (3, 3, 16), (2, 2, 64), (3, 3, 64),
+                                 (2, 2, 128)])
 @pytest.mark.parametrize("full_o3", [1, 0])
 def test_energy_forces_small_nets(lib, net, full_o3):
     """All (lmax, NL) plans incl. the unnatural-parity irreps of 3-layer full O(3); ragged widths; skin list."""
