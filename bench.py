@@ -211,7 +211,7 @@ def roofline_for(prof, stats, clocks, peaks, n_sm, n_atoms, ms_md_step):
     E_act, E_list = stats["active_edges"], stats["list_edges"]
     chunks = max(1, stats.get("chunks", 1))
     shares = {k: round(v["ms"] / tot_ms, 4) for k, v in prof.items() if v["launches"] and k not in ("tp_mix", "tp_mix16")}
-    names = {"gemm": "k_gemm_chain", "gemm_f16s": "k_gemm_f16s", "tp_fwd": "k_tp_fwd3 / k_tpo_fwd", "tp_bwd": "k_tp_bwd3 / k_tpo_bwd"}
+    names = {"gemm": "k_gemm_chain", "gemm_f16s": "k_gemm_f16s", "tp_fwd": "k_tp_fwd3 / k_tpmix_fwd / k_tpo_fwd", "tp_bwd": "k_tp_bwd3 / k_tpo_bwd_ring"}
     roof = {"kernel": names.get(dom, dom), "shares": shares}
     flops = {k: prof[k]["work"] * E_act / chunks for k in ("gemm", "gemm_f16s", "tp_fwd", "tp_bwd", "tp_mix", "tp_mix16") if k in prof}
     traffic, traffic_src = None, None
@@ -235,6 +235,11 @@ def roofline_for(prof, stats, clocks, peaks, n_sm, n_atoms, ms_md_step):
     else:
         roof.update({"bound": "hbm", "achieved": None, "peak": hbm, "unit": "GB/s", "frac": None, "traffic": traffic,
                      "peak_source": "MEASURED_PEAKS.json" if peaks else "fallback"})
+    # the tensor-product kernels against the FP32 ALU peak (their coupling arithmetic only: the channel mixing some of them also
+    # run on tensor cores is counted in the tensor term below)
+    roof["tensor_product"] = {k: {"kernel": names[k], "bound": "alu", "achieved": flops[k] / (prof[k]["ms"] * 1e-3) / 1e12, "peak": fp32_peak,
+                                  "unit": "TFLOP/s", "frac": flops[k] / (prof[k]["ms"] * 1e-3) / 1e12 / fp32_peak, "share_of_step": shares.get(k)}
+                              for k in ("tp_fwd", "tp_bwd") if k in flops and prof[k]["ms"] > 0}
     # ---- per MD step: t_roof = max(F_gemm / P_tc, F_alu / P_fp32, B_alg / BW_hbm)
     t_tensor = ((flops.get("gemm", 0.0) + flops.get("tp_mix", 0.0)) / (peak_tf32x3 * 1e12) + (flops.get("gemm_f16s", 0.0) + flops.get("tp_mix16", 0.0)) / (peak_f16s * 1e12)) * 1e3
     t_alu = (flops.get("tp_fwd", 0.0) + flops.get("tp_bwd", 0.0)) / (fp32_peak * 1e12) * 1e3
