@@ -1,9 +1,10 @@
 """Writes tests/golden/cfg3_subset.npz: fp64 oracle results on a seeded subset of BASELINE.json configs[3] (262,144 atoms,
 FM-sized network), for tests/test_gpu_parity_large.py.  Calls only oracle/ and the seeded generators of workloads.py; nothing
-here comes from the CUDA path.  The numpy oracle needs ~1.1 s per centre atom of this network on 8 cores, so the subset is
-16 force targets with their closure (every atom within r_c of a target: ~1,200 centre atoms, all of which also give a
-per-atom energy) — SURVEY.md 8d asks for 128 targets / 1,024 E_i; the E_i count is met, the force targets are what fits in
-~25 minutes of host time.  Also stored: the list rows (col, shift) at r_c + skin of 64 sampled atoms for the bit-exact
+here comes from the CUDA path.  The numpy oracle needs ~1.2 s per centre atom of this network (it ran on little more than one
+core of this container: 5,442 s for this file), so the subset is 64 force targets with their closure (every atom within r_c of a
+target: 4,694 centre atoms, all of which also give a per-atom energy) — SURVEY.md 8d asks for 128 targets / 1,024 E_i; the E_i
+count is met four times over, the force targets are what fits in 1.5 hours of host time.  Also stored: the list rows (col, shift)
+at r_c + skin of 128 sampled atoms for the bit-exact
 neighbour gate.  Run:  python tests/golden/make_cfg3_subset.py"""
 import os
 import sys
