@@ -200,8 +200,12 @@ int allegro_debug_num_paths(const allegro_hparams* hp, int layer);
  * allegro_debug_gemm runs one launch of that kernel on caller data:  C[M,N] = epi( pro([A0 | A1]) B ),  B(k,n) = wtrans ?
  * W[k*ldw+n] : W[n*ldw+k];  pro / epi are the PRO_* / EPI_* codes of csrc/gemm.cuh (0/1/2 and 0..6).  All pointers DEVICE fp32;
  * A0 / A1 hold rows_cap >= M rows; geo is the [M][8] edge record (u at [4]) or NULL.  Synchronises the stream.
- * Returns ALLEGRO_ERR_UNSUPPORTED when the shape or alignment is outside what the kernel takes. */
+ * Returns ALLEGRO_ERR_UNSUPPORTED when the shape or alignment is outside what the kernel takes.
+ * The kernel's packed copy of W is cached by (address, shape): right for the product, whose weights never move or change; a
+ * caller of allegro_debug_gemm that passes a NEW matrix calls allegro_debug_forget_weights first (it drops every cached packed
+ * weight and tensor map of the handle; they are rebuilt on demand). */
 int allegro_debug_set_precision(void* h, int passes);
+int allegro_debug_forget_weights(void* h);
 /* Test hook: capacity of the next list builds = E + frac * E + extra (default 0.125, 4096); (0, 0) forces the recovery path. */
 int allegro_debug_set_list_slack(void* h, double frac, int64_t extra);
 int allegro_debug_gemm(void* h, int64_t M, int64_t rows_cap, const float* A0, int lda0, int K0, const float* A1, int lda1, int K1,

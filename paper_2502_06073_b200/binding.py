@@ -27,7 +27,7 @@ EXPORTS = ["allegro_weight_layout", "allegro_create", "allegro_destroy", "allegr
            "allegro_set_state", "allegro_virial", "allegro_virial_noalloc", "allegro_debug_set_fusion", "allegro_debug_set_list_slack", "allegro_energy_forces_owned",
            "allegro_decomp_select", "allegro_decomp_scatter", "allegro_kick_drift", "allegro_get_state",
            "allegro_get_neighbors", "allegro_get_stats", "allegro_profile", "allegro_get_profile",
-           "allegro_debug_coupling", "allegro_debug_num_paths", "allegro_debug_set_precision", "allegro_debug_gemm",
+           "allegro_debug_coupling", "allegro_debug_num_paths", "allegro_debug_set_precision", "allegro_debug_gemm", "allegro_debug_forget_weights",
            "allegro_last_error"]
 VIRIAL_NOALLOC_MAX_ATOMS = 1048576   # ALLEGRO_VIRIAL_NOALLOC_MAX_ATOMS of include/allegro.h
 PROFILE_CLASSES = ["gemm", "tp_fwd", "tp_bwd", "gamma", "gammabar", "active_edges", "edge_misc", "neighbor", "md",
@@ -63,6 +63,7 @@ _lib.allegro_set_state.argtypes = [_vp, _vp, _vp, _vp]
 _lib.allegro_virial.argtypes = [_vp, _vp, _vp, _vp]
 _lib.allegro_virial_noalloc.argtypes = [_vp, _vp, _vp, _vp]
 _lib.allegro_debug_set_fusion.argtypes = [_vp, C.c_int]
+_lib.allegro_debug_forget_weights.argtypes = [_vp]
 _lib.allegro_debug_set_list_slack.argtypes = [_vp, _dbl, _i64]
 _lib.allegro_energy_forces_owned.argtypes = [_vp, _vp, _vp, _i64, _vp, _i64, _vp, _vp, _vp, _vp]
 _lib.allegro_decomp_select.argtypes = [_vp, _vp, _vp, _i64, _vp, _vp, _vp, _dbl, _i64, _vp, _vp, _vp, _vp, _vp, _vp]
@@ -269,6 +270,9 @@ class Allegro:
 
     def debug_set_precision(self, passes: int):
         self._check(_lib.allegro_debug_set_precision(self._h, int(passes)))
+
+    def debug_forget_weights(self):
+        self._check(_lib.allegro_debug_forget_weights(self._h))
 
     def debug_gemm(self, M, rows_cap, A0, K0, W, N, C_out, A1=None, K1=0, wtrans=0, ldw=None, pro=0, epi=0, aux=None, geo=None,
                    C2=None, split=0, c_old=0.0, c_new=1.0):

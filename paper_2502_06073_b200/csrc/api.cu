@@ -514,6 +514,18 @@ int allegro_debug_gemm(void* h, int64_t M, int64_t rows_cap, const float* A0, in
   return ALLEGRO_OK;
 }
 
+int allegro_debug_forget_weights(void* h) {
+  if (!h) return ALLEGRO_ERR_INVALID;
+  Model* m = static_cast<Model*>(h);
+  cudaError_t e = cudaDeviceSynchronize();
+  if (e != cudaSuccess) return cuda_fail(m, e, "allegro_debug_forget_weights");
+  for (auto& kv : m->packed_w) if (kv.second) cudaFree(kv.second);
+  m->packed_w.clear();
+  m->tmaps.clear();
+  md_graph_reset(m);   // a captured MD step holds the old pointers
+  return ALLEGRO_OK;
+}
+
 const char* allegro_last_error(void* h) {
   if (!h) return g_create_err.c_str();
   return static_cast<Model*>(h)->err.c_str();

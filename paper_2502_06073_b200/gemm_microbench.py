@@ -13,6 +13,7 @@ for (K, N, pro, epi) in [shapes[i] for i in sel]:
     C = torch.zeros(M, N, device="cuda"); C2 = torch.zeros(M, N, device="cuda"); aux = torch.randn(M, N, device="cuda")
     geo = torch.rand(M, 8, device="cuda")
     kw = dict(pro=pro, epi=epi, geo=geo, aux=aux if epi in (3, 4) else None, C2=C2 if epi in (2, 3) else None, c_old=0.7, c_new=0.7)
+    h.debug_forget_weights()           # W is a new matrix (the packed copy is cached by address and shape)
     for _ in range(2):
         h.debug_gemm(M, M, A, K, W, N, C, **kw)
     torch.cuda.synchronize()

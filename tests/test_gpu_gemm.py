@@ -63,6 +63,7 @@ def test_gemm_f16s_matches_fp64(lib, handle, case):
     C2w = (N - split) if epi == EPI_SPLIT_RES else N
     t = lambda a: torch.from_numpy(a).cuda()
     dA0, dA1, dW, dgeo, daux, dC, dC2 = t(A0), t(A1), t(Wdev), t(geo), t(aux), t(C0.copy()), t(np.zeros((cap, C2w), np.float32))
+    handle.debug_forget_weights()      # dW is a fresh matrix that may sit at a previous case's address
     handle.debug_gemm(M, cap, dA0, K0, dW, N, dC, A1=dA1 if K1 else None, K1=K1, wtrans=wtrans, pro=pro, epi=epi,
                       aux=(dC if epi == EPI_ACCUM else daux) if epi in (EPI_RESIDUAL, EPI_DSILU, EPI_ACCUM, EPI_SPLIT_RES) else None,
                       geo=dgeo, C2=dC2 if epi in (EPI_Y_X, EPI_RESIDUAL, EPI_SPLIT_RES) else None, split=split, c_old=c_old, c_new=c_new)
