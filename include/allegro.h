@@ -195,8 +195,9 @@ int allegro_debug_coupling(int l1, int l2, int l3, double* out);
 int allegro_debug_num_paths(const allegro_hparams* hp, int layer);
 
 /* Test hooks for the split-fp16 tcgen05 GEMM of the wide linears (csrc/gemm_f16s.cu; PAPER.md:93 / Table 1 MLPs).
- * allegro_debug_set_precision: 3 (default) = hi*hi + hi*lo + lo*hi, 2 = activations split only, 1 = plain fp16 — the
- * 1/2-pass kinds exist only for the committed precision study (R4).
+ * allegro_debug_set_precision: 3 (default) = the full split a_hi b_hi + a_hi b_lo + a_lo b_b (3 x TF32 hi*hi + hi*lo + lo*hi in the
+ * chained kernels), 2 = activations split only, 1 = one plain pass — the 1/2-pass kinds exist only for the committed precision
+ * study (R4, profiles/r2_precision.md).
  * allegro_debug_gemm runs one launch of that kernel on caller data:  C[M,N] = epi( pro([A0 | A1]) B ),  B(k,n) = wtrans ?
  * W[k*ldw+n] : W[n*ldw+k];  pro / epi are the PRO_* / EPI_* codes of csrc/gemm.cuh (0/1/2 and 0..6).  All pointers DEVICE fp32;
  * A0 / A1 hold rows_cap >= M rows; geo is the [M][8] edge record (u at [4]) or NULL.  Synchronises the stream.
