@@ -163,3 +163,34 @@ def test_cfg1_md_energy_conservation(lib):
 def test_cfg2_md_snapshots(lib):
     drift, bound, st = _md_snapshots(lib, WL.get(2), 60, 3, 22)       # shortened from the 1,000 steps of BASELINE.json
     print("cfg2 MD: |dE_tot| = %.3e eV (dt^2 bound %.3e)" % (drift, bound))
+
+
+def test_cfg3_md_conserves_energy_and_momentum(lib):
+    """6 NVE steps of BASELINE.json configs[3] (262,144 atoms, FM-sized network; the oracle cannot follow at this size: one of its
+    force evaluations is a day of host time, its forces on this config are checked at t = 0 from the cached subset above).  What holds
+    at any size: |E_tot(t) - E_tot(0)| <= (dt^2 / 8) max_t |sum_i F_i . a_i| (see _md_snapshots), total momentum stays at its
+    initial value (forces sum to zero: every edge contributes +g and -g), and every force is finite."""
+    import torch
+    w = WL.get(3)
+    g = lib.Allegro(lib.build_weights(w.hp, w.weight_seed), w.hp)
+    vel = WL.maxwell_boltzmann(w.mass, w.temperature, w.vel_seed)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    g.md_init(dev(w.pos), dev(vel), dev(w.mass.astype(np.float64)), dev(w.species.astype(np.int32)), w.cell, w.hp["r_cut"], w.skin)
+    N = w.n_atoms
+    v = torch.empty((N, 3), dtype=torch.float64, device="cuda"); F = torch.empty_like(v)
+    Ep = torch.empty(1, dtype=torch.float64, device="cuda"); Ek = torch.empty_like(Ep)
+    etot, bound = [], 0.0
+    p0 = (w.mass[:, None] * vel).sum(0)
+    for k in range(3):
+        if k:
+            g.md_step(w.dt_fs, 3)
+        g.get_state(vel=v, F=F, E_pot=Ep, E_kin=Ek)
+        f, vv = F.cpu().numpy(), v.cpu().numpy()
+        assert np.isfinite(f).all()
+        etot.append(float(Ep.item() + Ek.item()))
+        bound = max(bound, 0.125 * w.dt_fs ** 2 * abs(float((f * (O.ACC_CONV * f / w.mass[:, None])).sum())))
+        assert np.abs(f.sum(0)).max() <= 1e-6 * np.abs(f).sum(0).max()              # net force: fp32 edge terms summed in fp64
+        assert np.abs((w.mass[:, None] * vv).sum(0) - p0).max() <= 1e-6 * (w.mass[:, None] * np.abs(vv)).sum(0).max()
+    drift = max(abs(e - etot[0]) for e in etot)
+    print("cfg3 MD: |dE_tot| = %.3e eV over 6 steps (dt^2 bound %.3e), E_tot = %.6f eV" % (drift, bound, etot[0]))
+    assert drift <= bound, (etot, bound)
